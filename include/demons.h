@@ -1,0 +1,171 @@
+/* include/demons.h -- C ABI of the B200-native demons deformable-registration library.
+ *
+ * Method: Gu et al., "Implementation and evaluation of various demons deformable image
+ * registration algorithms on GPU" (arxiv/paper_0909_0928).  "PAPER.md L<n>" below is line n of
+ * the paper text; "reading Xn" refers to the ambiguity ledger in DESIGN.md.
+ *
+ * Conventions shared by every entry point
+ * ---------------------------------------
+ *  - All d_* pointers are DEVICE pointers (CUDA global memory of the current device), all h_*
+ *    pointers are HOST pointers.  The library never allocates device memory: the caller owns
+ *    every buffer and the workspace (demons_set_workspace), and they must stay alive until the
+ *    work enqueued on `stream` has completed.
+ *  - dims = {nx, ny, nz}.  A scalar volume is float32, flat index x + nx*(y + ny*z)
+ *    (Sec. 2.5: "x as rows, y as columns, z as frames" -- x is unit stride).
+ *  - A displacement field is float32, planar: component c (0 = x, 1 = y, 2 = z) starts at
+ *    base + c*nx*ny*nz.  Units are voxels of the level the field lives on (reading C3).
+ *  - Direction (reading C1): warp(I,u)(x) = trilinear(I, x + u(x)); the update is u <- u - F
+ *    with F exactly as printed in Eq.(1)-(6), d = Mw - S.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls
+ *    enqueue work on it and return without synchronising unless stated otherwise.
+ *  - Every function returns a DEMONS_* status; nothing throws, aborts or exits.  On failure
+ *    demons_last_error() returns a thread-local description.  There is no CPU fallback: with no
+ *    usable CUDA device every compute entry point returns DEMONS_E_CUDA.
+ *  - Pointers that are 16-byte aligned with nx % 4 == 0 take the 128-bit vectorised kernels;
+ *    anything else takes scalar kernels with identical results.
+ */
+#ifndef DEMONS_H
+#define DEMONS_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct demons_ctx demons_ctx;
+
+/* Variant k = the paper's "Method k+1" (Table 2). */
+enum {
+    DEMONS_PASSIVE = 0,            /* Eq.(1):  d gS / (d^2 + |gS|^2)                       */
+    DEMONS_EVOLVED_PASSIVE = 1,    /* Eq.(2), PAPER.md L64 (readings A3, A4), gS and gM0 fixed           */
+    DEMONS_ACTIVE = 2,             /* Eq.(3):  d gMw / (d^2 + |gMw|^2), gMw = grad(warp M) */
+    DEMONS_DOUBLE = 3,             /* Eq.(4):  Eq.(1) + Eq.(3)                             */
+    DEMONS_ADJUSTED_DOUBLE = 4,    /* Eq.(5), PAPER.md L93 (reading A5): alpha^2 d^2 in both denominators*/
+    DEMONS_INVERSE_CONSISTENT = 5  /* Eq.(6): G = gMw + gSw, d = Mw - Sw                  */
+};
+
+enum {
+    DEMONS_OK = 0,
+    DEMONS_E_ARG = -1,         /* NULL / out-of-range / inconsistent argument                 */
+    DEMONS_E_CUDA = -2,        /* a CUDA runtime call failed (no device, launch failure, ...) */
+    DEMONS_E_WORKSPACE = -3,   /* workspace missing or too small for this call                */
+    DEMONS_E_UNSUPPORTED = -4  /* valid request this build cannot serve (e.g. sigma too large) */
+};
+
+/* Largest Gaussian radius R = ceil(3 sigma) the smoothing kernels accept. */
+#define DEMONS_MAX_RADIUS 32
+/* Largest number of pyramid levels. */
+#define DEMONS_MAX_LEVELS 8
+/* Capacity of the per-iteration statistics buffer inside the workspace (rows of 3 doubles). */
+#define DEMONS_MAX_STATS_ROWS 16384
+
+/* ---- context ---------------------------------------------------------------------------
+ * demons_create: host-only, no CUDA call.  dims = finest-level volume size (each >= 1),
+ * spacing in mm (> 0; stored, used only by callers that report errors in mm, reading C3),
+ * variant in [0,5], alpha > 0 (used by variant 4 only), sigma > 0 in voxels
+ * with ceil(3 sigma) <= DEMONS_MAX_RADIUS ("Gaussian filter of unit standard deviation",
+ * PAPER.md L175; sigma is an argument per BASELINE.json north_star).
+ * The context holds host-side state only (parameters, workspace partition, cached CUDA graphs). */
+int demons_create(demons_ctx** out, const int dims[3], const float spacing[3], int variant,
+                  float alpha, float sigma);
+void demons_destroy(demons_ctx* ctx);
+
+/* Bytes of device workspace needed by every entry point below for volumes up to the context's
+ * dims and a pyramid of `levels` (1..DEMONS_MAX_LEVELS).  Includes the device staging buffers
+ * of demons_register_host.  Returns 0 on bad arguments. */
+size_t demons_workspace_bytes(const demons_ctx* ctx, int levels);
+/* d_ws: device pointer, 256-byte aligned, `bytes` >= demons_workspace_bytes(ctx, levels) for
+ * the `levels` later passed to demons_register.  The library zeroes its counters on `stream`
+ * lazily at first use.  The caller keeps ownership. */
+int demons_set_workspace(demons_ctx* ctx, void* d_ws, size_t bytes);
+
+/* Pyramid geometry (reading A12 / O6): level 0 = finest = ctx dims, level l+1 = ceil(level l / 2). */
+int demons_level_dims(const demons_ctx* ctx, int level, int out_dims[3]);
+
+/* Number of kernel launches this context has enqueued so far (graph replays count their nodes). */
+long long demons_launch_count(const demons_ctx* ctx);
+
+/* "profile" option: after a demons_register call made with the option on, the summed device time
+ * (ms, CUDA events on the caller's stream) and the number of timed groups per kernel class:
+ * [0] force kernels (fused warp+force+update, or the force pass of variants 2-5), [1] the warp
+ * pass of variants 2-5, [2] smoothing, [3] pyramid (restrict + prolong). */
+int demons_get_profile(const demons_ctx* ctx, double h_ms[4], long long h_launch_groups[4]);
+
+/* Named integer options.  "graphs" (default 1): replay the per-level iteration through a CUDA
+ * graph.  "texture" (default 0): S9, sample the moving image through the texture unit with
+ * hardware linear filtering (PAPER.md L181 reports its precision as insufficient; measured
+ * option only -- fails parity by design).  "generic_smooth" (default 0): always use
+ * the three separable smoothing passes instead of the fused kernel.  "profile" (default 0): time
+ * every kernel class with events inside demons_register (disables graphs, adds a final
+ * synchronise; see demons_get_profile).  Unknown name -> DEMONS_E_ARG. */
+int demons_set_option(demons_ctx* ctx, const char* name, int value);
+
+/* ---- full registration (PAPER.md L123-125 multi-scale, L145 stopping rule; O9/O10) ---------
+ * d_static, d_moving: finest-level volumes.  d_u: field of the moving image, [3][N];
+ * levels == 1: in = initial field, out = result; levels > 1: ignored on input (the coarsest
+ * level starts from zero), out = result.  d_u_back: variant 5 only (the field applied to the
+ * static image), same rule; must be NULL for the other variants.
+ * h_iters_per_level[levels], coarse -> fine, each >= 0, sum <= DEMONS_MAX_STATS_ROWS.
+ * eps <= 0: run exactly the given counts.  eps > 0: per level, stop after the first iteration
+ * n >= 10 with |l_n - l_{n-10}| <= eps, l_n = sum|F| / sum|u| (reading A13);
+ * tested on the device, no host round trip.
+ * h_stats (nullable): [sum iters][3] doubles = {SSD, sum|F|_2, sum|u|_2} per executed iteration
+ * in execution order, evaluated with the state before that iteration's update (reading O8); rows
+ * of skipped iterations are zero.  h_iters_done (nullable): [levels] iterations executed.
+ * If h_stats or h_iters_done is non-NULL the call synchronises `stream` before returning. */
+int demons_register(demons_ctx* ctx, const float* d_static, const float* d_moving, float* d_u,
+                    float* d_u_back, int levels, const int* h_iters_per_level, double eps,
+                    double* h_stats, int* h_iters_done, void* stream);
+
+/* Same, with HOST buffers: copies h_static/h_moving (and, for levels == 1, h_u / h_u_back) to
+ * staging buffers inside the workspace, registers, copies the field(s) back, synchronises.
+ * Pinned host memory makes the copies asynchronous on `stream`; pageable memory also works. */
+int demons_register_host(demons_ctx* ctx, const float* h_static, const float* h_moving, float* h_u,
+                         float* h_u_back, int levels, const int* h_iters_per_level, double eps,
+                         double* h_stats, int* h_iters_done, void* stream);
+
+/* ---- per-kernel entry points (one pass each, what the parity tests and the sweep call) -------
+ * All take explicit dims (nx*ny*nz must not exceed the context's finest volume).
+ *
+ * demons_warp_force: S1-S4 + S6 of the hot path -- Mw = warp(M, u_in) (software
+ * trilinear, L181), central-difference gradients (reading A7/A8), F per the context's variant
+ * (Eq.(1)-(6)), d_u_out = d_u_in - F, UNSMOOTHED.  Variant 5 also needs d_ub_in / d_ub_out
+ * (ub_out = ub_in + F); they must be NULL otherwise.  d_u_out must not alias any input.
+ * d_metrics (nullable): 3 doubles on the device = {SSD, sum|F|_2, sum|u_in|_2}. */
+int demons_warp_force(demons_ctx* ctx, const int dims[3], const float* d_static,
+                      const float* d_moving, const float* d_u_in, float* d_u_out,
+                      const float* d_ub_in, float* d_ub_out, double* d_metrics, void* stream);
+
+/* demons_smooth: S5 -- separable Gaussian of `ncomp` planar components, radius R = ceil(3 sigma),
+ * normalised taps, clamped borders (reading A9).  d_in != d_out. */
+int demons_smooth(demons_ctx* ctx, const int dims[3], const float* d_in, float* d_out, int ncomp,
+                  float sigma, void* stream);
+
+/* demons_restrict: S7 -- 2x2x2 box average to ceil(fine/2) ("down-sampled";
+ * reading A12).  d_coarse holds prod(ceil(fine_dims/2)) floats. */
+int demons_restrict(demons_ctx* ctx, const int fine_dims[3], const float* d_fine, float* d_coarse,
+                    void* stream);
+
+/* demons_prolong: S8 -- u_fine(x) = 2 * trilinear(u_coarse, clamp((x - 0.5)/2)), three planar
+ * components (one coarse voxel of motion = 2 fine voxels; reading A12). */
+int demons_prolong(demons_ctx* ctx, const int coarse_dims[3], const float* d_u_coarse,
+                   const int fine_dims[3], float* d_u_fine, void* stream);
+
+/* demons_ssd: the final SSD of O8 -- sum (warp(M,u) - S)^2, variant 5: sum (warp(M,u) -
+ * warp(S,ub))^2 (d_ub NULL otherwise).  d_out: 1 double on the device. */
+int demons_ssd(demons_ctx* ctx, const int dims[3], const float* d_static, const float* d_moving,
+               const float* d_u, const float* d_ub, double* d_out, void* stream);
+
+/* demons_ic_error: BASELINE.json config 4 -- e(x) = |u_f(x) + u_b(x + u_f(x))|_2, u_b sampled
+ * trilinearly with clamping (reading A14).  d_out: 2 doubles on the device = {mean e, max e}. */
+int demons_ic_error(demons_ctx* ctx, const int dims[3], const float* d_uf, const float* d_ub,
+                    double* d_out, void* stream);
+
+/* Thread-local description of the last failure on this thread ("" if none). */
+const char* demons_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DEMONS_H */

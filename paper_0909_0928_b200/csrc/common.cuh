@@ -1,0 +1,207 @@
+// Device-side helpers shared by the demons kernels (sm_100a).  Product code: nothing here is
+// shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace demons {
+
+struct Dims {
+    int nx, ny, nz;
+};
+
+__host__ __device__ __forceinline__ size_t nvox(const Dims& d) {
+    return (size_t)d.nx * (size_t)d.ny * (size_t)d.nz;
+}
+
+// Where the three metrics of one warp_force pass go (S6 of the hot path).
+// Per-block partials in double, fixed-order final sum by the last block to finish: the result
+// does not depend on scheduling.
+struct MetricSink {
+    double* partials;           // [nvals][stride] block partials
+    unsigned int* ticket;       // block-completion counter, left at 0 by the last block
+    double* out;                // nullptr: metrics not wanted
+    unsigned int* row_counter;  // nullable: the last block writes out[3*row..] and bumps *row_counter
+    int stride;                 // capacity of one partial row (>= number of blocks)
+    // device-side stopping rule (reading A13); all nullable / eps <= 0 = off
+    double* lhist;              // ring of relative norms l_n for this level, [LHIST]
+    int* lvalid;                // l_n defined (sum|u| > 0), [LHIST]
+    unsigned int* level_iter;   // iterations executed on this level
+    int* stop_force;            // set to 1 when the rule fires; force kernels then skip
+    int* stop_smooth;           // set by the first skipped force kernel; smoothing then skips
+    double eps;
+};
+
+constexpr int LHIST = 16;  // power of two >= 11 (lag of 10 iterations)
+
+__device__ __forceinline__ float lerpf(float a, float b, float t) { return fmaf(t, b - a, a); }
+
+// One axis of O2 (reading A11): p = x + u clamped to [0, n-1], i0 = floor(p), f = p - i0,
+// i1 = min(i0 + 1, n - 1).  The split is taken on u, not on x + u: floor(x + u) = x + floor(u)
+// for integer x and u - floor(u) is exact in fp32, so no bits of the fraction are lost to the
+// magnitude of x.
+__device__ __forceinline__ void split_axis(int x, float u, int n, int& i0, int& i1, float& f) {
+    float fl = floorf(u);
+    f = u - fl;
+    fl = fminf(fmaxf(fl, -16777216.f), 16777216.f);
+    int i = x + (int)fl;
+    if (i < 0) {
+        i = 0;
+        f = 0.f;
+    }
+    if (i >= n - 1) {
+        i = n - 1;
+        f = 0.f;
+    }
+    i0 = i;
+    i1 = min(i + 1, n - 1);
+}
+
+// Software trilinear sample of I at (x + ux, y + uy, z + uz): PAPER.md L179-181 ("our own
+// trilinear interpolation function").  Interpolates along x, then y, then z.
+__device__ __forceinline__ float trilinear(const float* __restrict__ I, const Dims& d, int x, int y,
+                                           int z, float ux, float uy, float uz) {
+    int x0, x1, y0, y1, z0, z1;
+    float fx, fy, fz;
+    split_axis(x, ux, d.nx, x0, x1, fx);
+    split_axis(y, uy, d.ny, y0, y1, fy);
+    split_axis(z, uz, d.nz, z0, z1, fz);
+    const float* p00 = I + ((size_t)z0 * d.ny + y0) * d.nx;
+    const float* p10 = I + ((size_t)z0 * d.ny + y1) * d.nx;
+    const float* p01 = I + ((size_t)z1 * d.ny + y0) * d.nx;
+    const float* p11 = I + ((size_t)z1 * d.ny + y1) * d.nx;
+    const float c000 = __ldg(p00 + x0), c100 = __ldg(p00 + x1);
+    const float c010 = __ldg(p10 + x0), c110 = __ldg(p10 + x1);
+    const float c001 = __ldg(p01 + x0), c101 = __ldg(p01 + x1);
+    const float c011 = __ldg(p11 + x0), c111 = __ldg(p11 + x1);
+    const float a00 = lerpf(c000, c100, fx), a10 = lerpf(c010, c110, fx);
+    const float a01 = lerpf(c001, c101, fx), a11 = lerpf(c011, c111, fx);
+    const float b0 = lerpf(a00, a10, fy), b1 = lerpf(a01, a11, fy);
+    return lerpf(b0, b1, fz);
+}
+
+// VEC consecutive floats along x: one 128-bit access when VEC == 4.
+template <int VEC>
+__device__ __forceinline__ void load_vec(const float* __restrict__ p, float (&v)[VEC]) {
+    if constexpr (VEC == 4) {
+        const float4 t = __ldg(reinterpret_cast<const float4*>(p));
+        v[0] = t.x;
+        v[1] = t.y;
+        v[2] = t.z;
+        v[3] = t.w;
+    } else {
+#pragma unroll
+        for (int j = 0; j < VEC; ++j) v[j] = __ldg(p + j);
+    }
+}
+
+template <int VEC>
+__device__ __forceinline__ void store_vec(float* __restrict__ p, const float (&v)[VEC]) {
+    if constexpr (VEC == 4) {
+        *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
+    } else {
+#pragma unroll
+        for (int j = 0; j < VEC; ++j) p[j] = v[j];
+    }
+}
+
+// Centre values and central-difference gradient (O1: g_c = (I(x+e_c) - I(x-e_c))/2, indices
+// clamped; reading A7) of VEC consecutive voxels starting at (x0, y, z).
+template <int VEC>
+__device__ __forceinline__ void centre_and_gradient(const float* __restrict__ I, const Dims& d, int x0,
+                                                    int y, int z, float (&c)[VEC], float (&gx)[VEC],
+                                                    float (&gy)[VEC], float (&gz)[VEC]) {
+    const size_t plane = (size_t)d.nx * d.ny;
+    const float* row = I + (size_t)z * plane + (size_t)y * d.nx;
+    float ym[VEC], yp[VEC], zm[VEC], zp[VEC];
+    load_vec<VEC>(row + x0, c);
+    const float xm = __ldg(row + max(x0 - 1, 0));
+    const float xp = __ldg(row + min(x0 + VEC, d.nx - 1));
+    load_vec<VEC>(I + (size_t)z * plane + (size_t)max(y - 1, 0) * d.nx + x0, ym);
+    load_vec<VEC>(I + (size_t)z * plane + (size_t)min(y + 1, d.ny - 1) * d.nx + x0, yp);
+    load_vec<VEC>(I + (size_t)max(z - 1, 0) * plane + (size_t)y * d.nx + x0, zm);
+    load_vec<VEC>(I + (size_t)min(z + 1, d.nz - 1) * plane + (size_t)y * d.nx + x0, zp);
+#pragma unroll
+    for (int j = 0; j < VEC; ++j) {
+        const float l = j > 0 ? c[j - 1] : xm;
+        const float r = j < VEC - 1 ? c[j + 1] : xp;
+        gx[j] = 0.5f * (r - l);
+        gy[j] = 0.5f * (yp[j] - ym[j]);
+        gz[j] = 0.5f * (zp[j] - zm[j]);
+    }
+}
+
+// q(num, den) = den > 1e-9 ? num/den : 0 -- the zero guard of reading A6.
+__device__ __forceinline__ float guarded_div(float num, float den) {
+    return den > 1e-9f ? __fdividef(num, den) : 0.f;
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+    return v;
+}
+
+// Block-wide reduction of NV doubles (sum; the last NMAX of them by max), publication of the
+// block partial, and the fixed-order final reduction by the last block to arrive.  Returns true
+// in thread 0 of the last block, with the totals in v.  Must be called by every thread.
+template <int NV, int NMAX = 0>
+__device__ __forceinline__ bool block_reduce_publish(double (&v)[NV], double* partials, int stride,
+                                                     unsigned int* ticket) {
+    __shared__ double sm[NV][32];
+    __shared__ int s_last;
+    const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+    const int nthreads = blockDim.x * blockDim.y * blockDim.z;
+    const int lane = tid & 31, wid = tid >> 5, nwarps = (nthreads + 31) >> 5;
+    const unsigned int nblocks = gridDim.x * gridDim.y * gridDim.z;
+    const unsigned int bid = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+        const double r = i >= NV - NMAX ? warp_max(v[i]) : warp_sum(v[i]);
+        if (lane == 0) sm[i][wid] = r;
+    }
+    __syncthreads();
+    if (wid == 0) {
+#pragma unroll
+        for (int i = 0; i < NV; ++i) {
+            double r = lane < nwarps ? sm[i][lane] : (i >= NV - NMAX ? -1.0e300 : 0.0);
+            r = i >= NV - NMAX ? warp_max(r) : warp_sum(r);
+            if (lane == 0) partials[(size_t)i * stride + bid] = r;
+        }
+        if (lane == 0) {
+            __threadfence();
+            const unsigned int t = atomicAdd(ticket, 1u);
+            s_last = (t == nblocks - 1u);
+        }
+    }
+    __syncthreads();
+    if (!s_last) return false;
+    __threadfence();
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+        const bool is_max = i >= NV - NMAX;
+        double r = is_max ? -1.0e300 : 0.0;
+        const volatile double* p = partials + (size_t)i * stride;
+        for (unsigned int b = tid; b < nblocks; b += nthreads) r = is_max ? fmax(r, p[b]) : r + p[b];
+        r = is_max ? warp_max(r) : warp_sum(r);
+        __syncthreads();  // sm[][] reuse
+        if (lane == 0) sm[i][wid] = r;
+        __syncthreads();
+        if (wid == 0) {
+            double q = lane < nwarps ? sm[i][lane] : (is_max ? -1.0e300 : 0.0);
+            q = is_max ? warp_max(q) : warp_sum(q);
+            v[i] = q;
+        }
+    }
+    if (tid == 0) *ticket = 0u;
+    return tid == 0;
+}
+
+}  // namespace demons

@@ -1,0 +1,739 @@
+// C ABI of the demons library (include/demons.h): context, workspace partition, the multi-scale
+// registration driver and the per-kernel entry points.
+#include "../../include/demons.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "kernels.h"
+
+using namespace demons;
+
+namespace {
+
+thread_local std::string g_last_error;
+
+int fail(int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_last_error = buf;
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                        \
+    do {                                                                                      \
+        cudaError_t e_ = (expr);                                                              \
+        if (e_ != cudaSuccess)                                                                \
+            return fail(DEMONS_E_CUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e_), \
+                        __FILE__, __LINE__);                                                  \
+    } while (0)
+
+constexpr size_t ALIGN = 256;
+size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
+
+// control block at the start of the workspace
+struct Control {
+    unsigned int ticket;       // 0
+    unsigned int row_counter;  // 4
+    unsigned int level_iter;   // 8
+    int stop_force;            // 12
+    int stop_smooth;           // 16
+    int pad0[11];              // -> 64
+    int lvalid[LHIST];         // 64
+    double lhist[LHIST];       // 128
+    int iters_done[DEMONS_MAX_LEVELS];  // 256
+    int pad1[56];
+};
+static_assert(sizeof(Control) == 512, "control block layout");
+
+struct Partition {
+    size_t control, partials, stats, Mw, Sw, uprime, ubprime, smooth_tmp;
+    size_t pyrS[DEMONS_MAX_LEVELS], pyrM[DEMONS_MAX_LEVELS], pyrU[DEMONS_MAX_LEVELS], pyrUb[DEMONS_MAX_LEVELS];
+    size_t hS, hM, hU, hUb;
+    size_t total;
+    int partial_stride;
+};
+
+struct GraphEntry {
+    Dims d;
+    const float *S, *M;
+    float *u, *ub;
+    int chunk;
+    double eps;
+    cudaGraphExec_t exec;
+    int launches;
+};
+
+}  // namespace
+
+struct demons_ctx {
+    Dims dims;
+    float spacing[3];
+    int variant;
+    float alpha;
+    float sigma;
+    char* ws = nullptr;
+    size_t ws_bytes = 0;
+    long long launches = 0;
+    int opt_graphs = 1;
+    int opt_texture = 0;
+    int opt_generic_smooth = 0;
+    int opt_profile = 0;
+    std::vector<cudaEvent_t> prof_all;                               // events of the profiled call
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_pairs[4];  // per kernel class: start/stop
+    double prof_ms[4] = {0, 0, 0, 0};
+    long long prof_n[4] = {0, 0, 0, 0};
+    std::vector<GraphEntry> graphs;
+    cudaArray_t tex_array = nullptr;
+    cudaTextureObject_t tex = 0;
+    Dims tex_dims{0, 0, 0};
+};
+
+namespace {
+
+Dims coarser(const Dims& d) { return Dims{(d.nx + 1) / 2, (d.ny + 1) / 2, (d.nz + 1) / 2}; }
+
+bool is_ic(const demons_ctx* c) { return c->variant == DEMONS_INVERSE_CONSISTENT; }
+
+// Gaussian taps (reading A9): R = ceil(3 sigma), w_k = exp(-k^2/2 sigma^2) / sum_j exp(-j^2/2 sigma^2),
+// evaluated in double and rounded to float.
+int gaussian_taps(double sigma, float* w) {
+    const int R = (int)std::ceil(3.0 * sigma);
+    if (R < 0 || R > DEMONS_MAX_RADIUS) return -1;
+    double e[DEMONS_MAX_RADIUS + 1];
+    double total = 0.0;
+    for (int k = 0; k <= R; ++k) {
+        e[k] = std::exp(-0.5 * (double)k * (double)k / (sigma * sigma));
+        total += k == 0 ? e[k] : 2.0 * e[k];
+    }
+    for (int k = 0; k <= R; ++k) w[k] = (float)(e[k] / total);
+    return R;
+}
+
+Partition make_partition(const demons_ctx* c, int levels) {
+    Partition p{};
+    const size_t N = nvox(c->dims);
+    const bool ic = is_ic(c);
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        const size_t o = off;
+        off += align_up(bytes);
+        return o;
+    };
+    p.control = take(sizeof(Control));
+    int stride = force_partial_blocks(c->dims);
+    if (stride < 148 * 8) stride = 148 * 8;
+    p.partial_stride = stride;
+    p.partials = take(3 * (size_t)stride * sizeof(double));
+    p.stats = take((size_t)DEMONS_MAX_STATS_ROWS * 3 * sizeof(double));
+    p.Mw = take(N * 4);
+    p.Sw = ic ? take(N * 4) : 0;
+    p.uprime = take(3 * N * 4);
+    p.ubprime = ic ? take(3 * N * 4) : 0;
+    p.smooth_tmp = take(N * 4);
+    Dims d = c->dims;
+    for (int l = 1; l < levels; ++l) {
+        d = coarser(d);
+        const size_t n = nvox(d);
+        p.pyrS[l] = take(n * 4);
+        p.pyrM[l] = take(n * 4);
+        p.pyrU[l] = take(3 * n * 4);
+        p.pyrUb[l] = ic ? take(3 * n * 4) : 0;
+    }
+    p.hS = take(N * 4);
+    p.hM = take(N * 4);
+    p.hU = take(3 * N * 4);
+    p.hUb = ic ? take(3 * N * 4) : 0;
+    p.total = off;
+    return p;
+}
+
+bool dims_ok(const int dims[3]) {
+    if (!dims) return false;
+    for (int c = 0; c < 3; ++c)
+        if (dims[c] < 1 || dims[c] > 16384) return false;
+    const double n = (double)dims[0] * dims[1] * dims[2];
+    return n < 2147483647.0 / 4.0;
+}
+
+int check_ws(const demons_ctx* c, int levels) {
+    if (!c->ws) return fail(DEMONS_E_WORKSPACE, "no workspace set (demons_set_workspace)");
+    const Partition p = make_partition(c, levels);
+    if (p.total > c->ws_bytes)
+        return fail(DEMONS_E_WORKSPACE, "workspace too small: have %zu bytes, need %zu for %d level(s)",
+                    c->ws_bytes, p.total, levels);
+    return DEMONS_OK;
+}
+
+int check_call_dims(const demons_ctx* c, const int dims[3], Dims* out) {
+    if (!dims_ok(dims)) return fail(DEMONS_E_ARG, "bad dims");
+    const Dims d{dims[0], dims[1], dims[2]};
+    if (nvox(d) > nvox(c->dims))
+        return fail(DEMONS_E_WORKSPACE, "volume %dx%dx%d exceeds the context's %dx%dx%d", d.nx, d.ny, d.nz,
+                    c->dims.nx, c->dims.ny, c->dims.nz);
+    *out = d;
+    return DEMONS_OK;
+}
+
+MetricSink make_sink(const demons_ctx* c, const Partition& p, double* out, bool driver, double eps) {
+    MetricSink s{};
+    Control* ctl = reinterpret_cast<Control*>(c->ws + p.control);
+    s.partials = reinterpret_cast<double*>(c->ws + p.partials);
+    s.ticket = &ctl->ticket;
+    s.out = out;
+    s.stride = p.partial_stride;
+    if (driver) {
+        s.row_counter = &ctl->row_counter;
+        s.lhist = ctl->lhist;
+        s.lvalid = ctl->lvalid;
+        s.level_iter = &ctl->level_iter;
+        s.stop_force = &ctl->stop_force;
+        s.stop_smooth = &ctl->stop_smooth;
+        s.eps = eps;
+    }
+    return s;
+}
+
+void release_texture(demons_ctx* c) {
+    if (c->tex) cudaDestroyTextureObject(c->tex);
+    if (c->tex_array) cudaFreeArray(c->tex_array);
+    c->tex = 0;
+    c->tex_array = nullptr;
+}
+
+// S9 (measured option): copy M into a 3D CUDA array and bind it with hardware linear filtering,
+// clamp addressing ("map the original static images and moving images on the texture
+// memory").  The array is the one device allocation the library makes itself (a cudaArray cannot be
+// a torch tensor); it lives in the context.
+int bind_texture(demons_ctx* c, const Dims& d, const float* M, cudaStream_t st) {
+    if (!c->tex_array || c->tex_dims.nx != d.nx || c->tex_dims.ny != d.ny || c->tex_dims.nz != d.nz) {
+        release_texture(c);
+        cudaChannelFormatDesc fmt = cudaCreateChannelDesc<float>();
+        CUDA_TRY(cudaMalloc3DArray(&c->tex_array, &fmt, make_cudaExtent(d.nx, d.ny, d.nz)));
+        cudaResourceDesc rd{};
+        rd.resType = cudaResourceTypeArray;
+        rd.res.array.array = c->tex_array;
+        cudaTextureDesc td{};
+        td.addressMode[0] = td.addressMode[1] = td.addressMode[2] = cudaAddressModeClamp;
+        td.filterMode = cudaFilterModeLinear;
+        td.readMode = cudaReadModeElementType;
+        td.normalizedCoords = 0;
+        CUDA_TRY(cudaCreateTextureObject(&c->tex, &rd, &td, nullptr));
+        c->tex_dims = d;
+    }
+    cudaMemcpy3DParms cp{};
+    cp.srcPtr = make_cudaPitchedPtr(const_cast<float*>(M), (size_t)d.nx * 4, d.nx, d.ny);
+    cp.dstArray = c->tex_array;
+    cp.extent = make_cudaExtent(d.nx, d.ny, d.nz);
+    cp.kind = cudaMemcpyDeviceToDevice;
+    CUDA_TRY(cudaMemcpy3DAsync(&cp, st));
+    return DEMONS_OK;
+}
+
+enum { PROF_FORCE = 0, PROF_WARP = 1, PROF_SMOOTH = 2, PROF_PYRAMID = 3 };
+
+// "profile" option: bracket every launch of a kernel class with a pair of events on the stream.
+cudaEvent_t prof_event(demons_ctx* c, cudaStream_t st, bool record) {
+    if (!c->opt_profile) return nullptr;
+    cudaEvent_t e = nullptr;
+    if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
+    if (record) cudaEventRecord(e, st);
+    c->prof_all.push_back(e);
+    return e;
+}
+
+void prof_pair(demons_ctx* c, int cls, cudaEvent_t a, cudaEvent_t b) {
+    if (a && b) c->prof_pairs[cls].push_back({a, b});
+}
+
+void prof_clear(demons_ctx* c) {
+    for (cudaEvent_t e : c->prof_all) cudaEventDestroy(e);
+    c->prof_all.clear();
+    for (int k = 0; k < 4; ++k) c->prof_pairs[k].clear();
+}
+
+void prof_collect(demons_ctx* c) {  // after a stream synchronise
+    for (int k = 0; k < 4; ++k) {
+        double ms = 0.0;
+        for (auto& pr : c->prof_pairs[k]) {
+            float t = 0.f;
+            if (cudaEventElapsedTime(&t, pr.first, pr.second) == cudaSuccess) ms += t;
+        }
+        c->prof_ms[k] = ms;
+        c->prof_n[k] = (long long)c->prof_pairs[k].size();
+    }
+    prof_clear(c);
+}
+
+struct LevelBuffers {
+    Dims d;
+    const float* S;
+    const float* M;
+    float* u;
+    float* ub;
+};
+
+// One iteration: [warp_force ; smooth the total field] (reading C2).
+int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb, double eps, cudaStream_t st,
+                      int* launches) {
+    const bool ic = is_ic(c);
+    ForceArgs fa{};
+    fa.d = lb.d;
+    fa.variant = c->variant;
+    fa.alpha2 = c->variant == DEMONS_ADJUSTED_DOUBLE ? c->alpha * c->alpha : 1.f;
+    fa.S = lb.S;
+    fa.M = lb.M;
+    fa.u_in = lb.u;
+    fa.u_out = reinterpret_cast<float*>(c->ws + p.uprime);
+    fa.ub_in = ic ? lb.ub : nullptr;
+    fa.ub_out = ic ? reinterpret_cast<float*>(c->ws + p.ubprime) : nullptr;
+    fa.Mw = reinterpret_cast<float*>(c->ws + p.Mw);
+    fa.Sw = ic ? reinterpret_cast<float*>(c->ws + p.Sw) : nullptr;
+    fa.sink = make_sink(c, p, reinterpret_cast<double*>(c->ws + p.stats), true, eps);
+    fa.texM = c->opt_texture ? c->tex : 0;
+    cudaEvent_t e0 = prof_event(c, st, true);
+    fa.ev_mid = c->variant >= DEMONS_ACTIVE ? prof_event(c, st, false) : nullptr;
+    int n = launch_warp_force(fa, st);
+    if (n < 0) return fail(DEMONS_E_CUDA, "warp_force launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    *launches += n;
+    cudaEvent_t e1 = prof_event(c, st, true);
+    if (fa.ev_mid) {
+        prof_pair(c, PROF_WARP, e0, fa.ev_mid);
+        prof_pair(c, PROF_FORCE, fa.ev_mid, e1);
+    } else {
+        prof_pair(c, PROF_FORCE, e0, e1);
+    }
+    SmoothArgs sa{};
+    sa.d = lb.d;
+    sa.tmp = reinterpret_cast<float*>(c->ws + p.smooth_tmp);
+    sa.ncomp = 3;
+    sa.R = gaussian_taps(c->sigma, sa.w);
+    sa.skip = &reinterpret_cast<Control*>(c->ws + p.control)->stop_smooth;
+    sa.force_generic = c->opt_generic_smooth;
+    sa.in = fa.u_out;
+    sa.out = lb.u;
+    n = launch_smooth(sa, st);
+    if (n < 0) return fail(DEMONS_E_CUDA, "smooth launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    *launches += n;
+    if (ic) {
+        sa.in = fa.ub_out;
+        sa.out = lb.ub;
+        n = launch_smooth(sa, st);
+        if (n < 0) return fail(DEMONS_E_CUDA, "smooth launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        *launches += n;
+    }
+    prof_pair(c, PROF_SMOOTH, e1, prof_event(c, st, true));
+    return DEMONS_OK;
+}
+
+bool capturable(cudaStream_t st) { return st != nullptr && st != cudaStreamLegacy; }
+
+int run_level(demons_ctx* c, const Partition& p, const LevelBuffers& lb, int iters, double eps, cudaStream_t st) {
+    int done = 0;
+    const int chunk = iters >= 20 ? 20 : iters;
+    if (c->opt_graphs && capturable(st) && iters >= 4 && !c->opt_texture && !c->opt_profile) {
+        GraphEntry* ge = nullptr;
+        for (auto& g : c->graphs)
+            if (g.d.nx == lb.d.nx && g.d.ny == lb.d.ny && g.d.nz == lb.d.nz && g.S == lb.S && g.M == lb.M &&
+                g.u == lb.u && g.ub == lb.ub && g.chunk == chunk && g.eps == eps)
+                ge = &g;
+        if (!ge) {
+            GraphEntry g{};
+            g.d = lb.d;
+            g.S = lb.S;
+            g.M = lb.M;
+            g.u = lb.u;
+            g.ub = lb.ub;
+            g.chunk = chunk;
+            g.eps = eps;
+            cudaGraph_t graph = nullptr;
+            CUDA_TRY(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+            int rc = DEMONS_OK;
+            for (int i = 0; i < chunk && rc == DEMONS_OK; ++i) rc = enqueue_iteration(c, p, lb, eps, st, &g.launches);
+            cudaError_t e = cudaStreamEndCapture(st, &graph);
+            if (rc != DEMONS_OK) {
+                if (graph) cudaGraphDestroy(graph);
+                return rc;
+            }
+            if (e != cudaSuccess) return fail(DEMONS_E_CUDA, "graph capture failed: %s", cudaGetErrorString(e));
+            e = cudaGraphInstantiate(&g.exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (e != cudaSuccess) return fail(DEMONS_E_CUDA, "graph instantiate failed: %s", cudaGetErrorString(e));
+            if (c->graphs.size() >= 32) {  // bounded cache
+                cudaGraphExecDestroy(c->graphs.front().exec);
+                c->graphs.erase(c->graphs.begin());
+            }
+            c->graphs.push_back(g);
+            ge = &c->graphs.back();
+        }
+        while (iters - done >= chunk) {
+            CUDA_TRY(cudaGraphLaunch(ge->exec, st));
+            c->launches += ge->launches;
+            done += chunk;
+        }
+    }
+    for (; done < iters; ++done) {
+        int n = 0;
+        const int rc = enqueue_iteration(c, p, lb, eps, st, &n);
+        if (rc != DEMONS_OK) return rc;
+        c->launches += n;
+    }
+    return DEMONS_OK;
+}
+
+int register_impl(demons_ctx* c, const float* dS, const float* dM, float* du, float* dub, int levels,
+                  const int* iters, double eps, double* h_stats, int* h_done, cudaStream_t st) {
+    const bool ic = is_ic(c);
+    const Partition p = make_partition(c, levels);
+    Control* ctl = reinterpret_cast<Control*>(c->ws + p.control);
+    long long total_iters = 0;
+    for (int l = 0; l < levels; ++l) total_iters += iters[l];
+    prof_clear(c);
+    CUDA_TRY(cudaMemsetAsync(ctl, 0, sizeof(Control), st));
+    if (total_iters > 0) CUDA_TRY(cudaMemsetAsync(c->ws + p.stats, 0, (size_t)total_iters * 24, st));
+
+    // pyramids (O6): images only, no pre-blur (reading A15)
+    LevelBuffers lb[DEMONS_MAX_LEVELS];
+    lb[0] = LevelBuffers{c->dims, dS, dM, du, dub};
+    for (int l = 1; l < levels; ++l) {
+        lb[l].d = coarser(lb[l - 1].d);
+        float* s = reinterpret_cast<float*>(c->ws + p.pyrS[l]);
+        float* m = reinterpret_cast<float*>(c->ws + p.pyrM[l]);
+        lb[l].S = s;
+        lb[l].M = m;
+        lb[l].u = reinterpret_cast<float*>(c->ws + p.pyrU[l]);
+        lb[l].ub = ic ? reinterpret_cast<float*>(c->ws + p.pyrUb[l]) : nullptr;
+        cudaEvent_t e0 = prof_event(c, st, true);
+        if (launch_restrict(lb[l - 1].d, lb[l - 1].S, s, st) < 0 || launch_restrict(lb[l - 1].d, lb[l - 1].M, m, st) < 0)
+            return fail(DEMONS_E_CUDA, "restrict launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        c->launches += 2;
+        prof_pair(c, PROF_PYRAMID, e0, prof_event(c, st, true));
+    }
+    if (levels > 1) {  // the coarsest level starts from zero (O9)
+        const size_t n = nvox(lb[levels - 1].d);
+        CUDA_TRY(cudaMemsetAsync(lb[levels - 1].u, 0, 3 * n * 4, st));
+        if (ic) CUDA_TRY(cudaMemsetAsync(lb[levels - 1].ub, 0, 3 * n * 4, st));
+    }
+    for (int step = 0; step < levels; ++step) {
+        const int l = levels - 1 - step;  // coarse -> fine
+        if (step > 0) CUDA_TRY(cudaMemsetAsync(&ctl->level_iter, 0, 12, st));  // level_iter, stop_force, stop_smooth
+        if (c->opt_texture) {
+            const int rc = bind_texture(c, lb[l].d, lb[l].M, st);
+            if (rc != DEMONS_OK) return rc;
+        }
+        const int rc = run_level(c, p, lb[l], iters[step], eps, st);
+        if (rc != DEMONS_OK) return rc;
+        CUDA_TRY(cudaMemcpyAsync(&ctl->iters_done[step], &ctl->level_iter, 4, cudaMemcpyDeviceToDevice, st));
+        if (l > 0) {  // O7
+            cudaEvent_t e0 = prof_event(c, st, true);
+            if (launch_prolong(lb[l].d, lb[l].u, lb[l - 1].d, lb[l - 1].u, st) < 0)
+                return fail(DEMONS_E_CUDA, "prolong launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+            c->launches += 1;
+            if (ic) {
+                if (launch_prolong(lb[l].d, lb[l].ub, lb[l - 1].d, lb[l - 1].ub, st) < 0)
+                    return fail(DEMONS_E_CUDA, "prolong launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+                c->launches += 1;
+            }
+            prof_pair(c, PROF_PYRAMID, e0, prof_event(c, st, true));
+        }
+    }
+    if (h_stats && total_iters > 0)
+        CUDA_TRY(cudaMemcpyAsync(h_stats, c->ws + p.stats, (size_t)total_iters * 24, cudaMemcpyDeviceToHost, st));
+    if (h_done) CUDA_TRY(cudaMemcpyAsync(h_done, ctl->iters_done, (size_t)levels * 4, cudaMemcpyDeviceToHost, st));
+    if (h_stats || h_done || c->opt_profile) CUDA_TRY(cudaStreamSynchronize(st));
+    if (c->opt_profile) prof_collect(c);
+    return DEMONS_OK;
+}
+
+int check_register_args(demons_ctx* c, const void* S, const void* M, const void* u, const void* ub, int levels,
+                        const int* iters) {
+    if (!c) return fail(DEMONS_E_ARG, "ctx is NULL");
+    if (!S || !M || !u) return fail(DEMONS_E_ARG, "static, moving and u must be non-NULL");
+    if (is_ic(c) && !ub) return fail(DEMONS_E_ARG, "variant 5 needs u_back");
+    if (!is_ic(c) && ub) return fail(DEMONS_E_ARG, "u_back must be NULL unless variant 5");
+    if (levels < 1 || levels > DEMONS_MAX_LEVELS) return fail(DEMONS_E_ARG, "levels out of range");
+    if (!iters) return fail(DEMONS_E_ARG, "iters_per_level is NULL");
+    long long total = 0;
+    for (int l = 0; l < levels; ++l) {
+        if (iters[l] < 0) return fail(DEMONS_E_ARG, "negative iteration count");
+        total += iters[l];
+    }
+    if (total > DEMONS_MAX_STATS_ROWS) return fail(DEMONS_E_ARG, "more than DEMONS_MAX_STATS_ROWS iterations");
+    return check_ws(c, levels);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* demons_last_error(void) { return g_last_error.c_str(); }
+
+int demons_create(demons_ctx** out, const int dims[3], const float spacing[3], int variant, float alpha,
+                  float sigma) {
+    if (!out) return fail(DEMONS_E_ARG, "out is NULL");
+    *out = nullptr;
+    if (!dims_ok(dims)) return fail(DEMONS_E_ARG, "dims must be in [1,16384] with fewer than 2^29 voxels");
+    if (!spacing || !(spacing[0] > 0.f) || !(spacing[1] > 0.f) || !(spacing[2] > 0.f))
+        return fail(DEMONS_E_ARG, "spacing must be positive");
+    if (variant < 0 || variant > 5) return fail(DEMONS_E_ARG, "variant must be 0..5");
+    if (!(alpha > 0.f) || !std::isfinite(alpha)) return fail(DEMONS_E_ARG, "alpha must be positive");
+    if (!(sigma > 0.f) || !std::isfinite(sigma)) return fail(DEMONS_E_ARG, "sigma must be positive");
+    float w[DEMONS_MAX_RADIUS + 1];
+    if (gaussian_taps(sigma, w) < 0)
+        return fail(DEMONS_E_UNSUPPORTED, "ceil(3 sigma) exceeds DEMONS_MAX_RADIUS (%d)", DEMONS_MAX_RADIUS);
+    demons_ctx* c = new (std::nothrow) demons_ctx();
+    if (!c) return fail(DEMONS_E_ARG, "out of host memory");
+    c->dims = Dims{dims[0], dims[1], dims[2]};
+    for (int i = 0; i < 3; ++i) c->spacing[i] = spacing[i];
+    c->variant = variant;
+    c->alpha = alpha;
+    c->sigma = sigma;
+    *out = c;
+    return DEMONS_OK;
+}
+
+void demons_destroy(demons_ctx* c) {
+    if (!c) return;
+    for (auto& g : c->graphs) cudaGraphExecDestroy(g.exec);
+    release_texture(c);
+    prof_clear(c);
+    delete c;
+}
+
+size_t demons_workspace_bytes(const demons_ctx* c, int levels) {
+    if (!c || levels < 1 || levels > DEMONS_MAX_LEVELS) return 0;
+    return make_partition(c, levels).total;
+}
+
+int demons_set_workspace(demons_ctx* c, void* d_ws, size_t bytes) {
+    if (!c || !d_ws) return fail(DEMONS_E_ARG, "ctx / workspace is NULL");
+    if (reinterpret_cast<uintptr_t>(d_ws) % ALIGN) return fail(DEMONS_E_ARG, "workspace must be 256-byte aligned");
+    if (bytes < make_partition(c, 1).total)
+        return fail(DEMONS_E_WORKSPACE, "workspace too small: %zu < %zu", bytes, make_partition(c, 1).total);
+    for (auto& g : c->graphs) cudaGraphExecDestroy(g.exec);
+    c->graphs.clear();
+    CUDA_TRY(cudaMemset(d_ws, 0, sizeof(Control)));
+    CUDA_TRY(cudaDeviceSynchronize());
+    c->ws = static_cast<char*>(d_ws);
+    c->ws_bytes = bytes;
+    return DEMONS_OK;
+}
+
+int demons_level_dims(const demons_ctx* c, int level, int out_dims[3]) {
+    if (!c || !out_dims || level < 0 || level >= DEMONS_MAX_LEVELS) return fail(DEMONS_E_ARG, "bad arguments");
+    Dims d = c->dims;
+    for (int l = 0; l < level; ++l) d = coarser(d);
+    out_dims[0] = d.nx;
+    out_dims[1] = d.ny;
+    out_dims[2] = d.nz;
+    return DEMONS_OK;
+}
+
+long long demons_launch_count(const demons_ctx* c) { return c ? c->launches : 0; }
+
+int demons_get_profile(const demons_ctx* c, double h_ms[4], long long h_launch_groups[4]) {
+    if (!c || !h_ms || !h_launch_groups) return fail(DEMONS_E_ARG, "bad arguments");
+    for (int k = 0; k < 4; ++k) {
+        h_ms[k] = c->prof_ms[k];
+        h_launch_groups[k] = c->prof_n[k];
+    }
+    return DEMONS_OK;
+}
+
+int demons_set_option(demons_ctx* c, const char* name, int value) {
+    if (!c || !name) return fail(DEMONS_E_ARG, "bad arguments");
+    if (!strcmp(name, "graphs")) c->opt_graphs = value != 0;
+    else if (!strcmp(name, "texture")) c->opt_texture = value != 0;
+    else if (!strcmp(name, "generic_smooth")) c->opt_generic_smooth = value != 0;
+    else if (!strcmp(name, "profile")) c->opt_profile = value != 0;
+    else return fail(DEMONS_E_ARG, "unknown option '%s'", name);
+    for (auto& g : c->graphs) cudaGraphExecDestroy(g.exec);
+    c->graphs.clear();
+    return DEMONS_OK;
+}
+
+int demons_register(demons_ctx* c, const float* d_static, const float* d_moving, float* d_u, float* d_u_back,
+                    int levels, const int* h_iters, double eps, double* h_stats, int* h_iters_done, void* stream) {
+    const int rc = check_register_args(c, d_static, d_moving, d_u, d_u_back, levels, h_iters);
+    if (rc != DEMONS_OK) return rc;
+    return register_impl(c, d_static, d_moving, d_u, d_u_back, levels, h_iters, eps, h_stats, h_iters_done,
+                         static_cast<cudaStream_t>(stream));
+}
+
+int demons_register_host(demons_ctx* c, const float* h_static, const float* h_moving, float* h_u, float* h_u_back,
+                         int levels, const int* h_iters, double eps, double* h_stats, int* h_iters_done,
+                         void* stream) {
+    const int rc = check_register_args(c, h_static, h_moving, h_u, h_u_back, levels, h_iters);
+    if (rc != DEMONS_OK) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const Partition p = make_partition(c, levels);
+    const size_t N = nvox(c->dims);
+    const bool ic = is_ic(c);
+    float* dS = reinterpret_cast<float*>(c->ws + p.hS);
+    float* dM = reinterpret_cast<float*>(c->ws + p.hM);
+    float* dU = reinterpret_cast<float*>(c->ws + p.hU);
+    float* dUb = ic ? reinterpret_cast<float*>(c->ws + p.hUb) : nullptr;
+    CUDA_TRY(cudaMemcpyAsync(dS, h_static, N * 4, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(dM, h_moving, N * 4, cudaMemcpyHostToDevice, st));
+    if (levels == 1) {
+        CUDA_TRY(cudaMemcpyAsync(dU, h_u, 3 * N * 4, cudaMemcpyHostToDevice, st));
+        if (ic) CUDA_TRY(cudaMemcpyAsync(dUb, h_u_back, 3 * N * 4, cudaMemcpyHostToDevice, st));
+    }
+    const int rr = register_impl(c, dS, dM, dU, dUb, levels, h_iters, eps, nullptr, nullptr, st);
+    if (rr != DEMONS_OK) return rr;
+    CUDA_TRY(cudaMemcpyAsync(h_u, dU, 3 * N * 4, cudaMemcpyDeviceToHost, st));
+    if (ic) CUDA_TRY(cudaMemcpyAsync(h_u_back, dUb, 3 * N * 4, cudaMemcpyDeviceToHost, st));
+    long long total_iters = 0;
+    for (int l = 0; l < levels; ++l) total_iters += h_iters[l];
+    Control* ctl = reinterpret_cast<Control*>(c->ws + p.control);
+    if (h_stats && total_iters > 0)
+        CUDA_TRY(cudaMemcpyAsync(h_stats, c->ws + p.stats, (size_t)total_iters * 24, cudaMemcpyDeviceToHost, st));
+    if (h_iters_done)
+        CUDA_TRY(cudaMemcpyAsync(h_iters_done, ctl->iters_done, (size_t)levels * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return DEMONS_OK;
+}
+
+int demons_warp_force(demons_ctx* c, const int dims[3], const float* d_static, const float* d_moving,
+                      const float* d_u_in, float* d_u_out, const float* d_ub_in, float* d_ub_out, double* d_metrics,
+                      void* stream) {
+    if (!c) return fail(DEMONS_E_ARG, "ctx is NULL");
+    Dims d;
+    int rc = check_call_dims(c, dims, &d);
+    if (rc != DEMONS_OK) return rc;
+    if (!d_static || !d_moving || !d_u_in || !d_u_out) return fail(DEMONS_E_ARG, "NULL volume / field pointer");
+    if (d_u_in == d_u_out) return fail(DEMONS_E_ARG, "u_out must not alias u_in");
+    const bool ic = is_ic(c);
+    if (ic && (!d_ub_in || !d_ub_out)) return fail(DEMONS_E_ARG, "variant 5 needs ub_in and ub_out");
+    if (!ic && (d_ub_in || d_ub_out)) return fail(DEMONS_E_ARG, "ub_in / ub_out must be NULL unless variant 5");
+    if (ic && d_ub_in == d_ub_out) return fail(DEMONS_E_ARG, "ub_out must not alias ub_in");
+    rc = check_ws(c, 1);
+    if (rc != DEMONS_OK) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const Partition p = make_partition(c, 1);
+    ForceArgs fa{};
+    fa.d = d;
+    fa.variant = c->variant;
+    fa.alpha2 = c->variant == DEMONS_ADJUSTED_DOUBLE ? c->alpha * c->alpha : 1.f;
+    fa.S = d_static;
+    fa.M = d_moving;
+    fa.u_in = d_u_in;
+    fa.u_out = d_u_out;
+    fa.ub_in = d_ub_in;
+    fa.ub_out = d_ub_out;
+    fa.Mw = reinterpret_cast<float*>(c->ws + p.Mw);
+    fa.Sw = ic ? reinterpret_cast<float*>(c->ws + p.Sw) : nullptr;
+    fa.sink = make_sink(c, p, d_metrics, false, 0.0);
+    if (c->opt_texture) {
+        rc = bind_texture(c, d, d_moving, st);
+        if (rc != DEMONS_OK) return rc;
+        fa.texM = c->tex;
+    }
+    const int n = launch_warp_force(fa, st);
+    if (n < 0) return fail(DEMONS_E_CUDA, "warp_force launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    c->launches += n;
+    return DEMONS_OK;
+}
+
+int demons_smooth(demons_ctx* c, const int dims[3], const float* d_in, float* d_out, int ncomp, float sigma,
+                  void* stream) {
+    if (!c) return fail(DEMONS_E_ARG, "ctx is NULL");
+    Dims d;
+    int rc = check_call_dims(c, dims, &d);
+    if (rc != DEMONS_OK) return rc;
+    if (!d_in || !d_out) return fail(DEMONS_E_ARG, "NULL field pointer");
+    if (d_in == d_out) return fail(DEMONS_E_ARG, "in-place smoothing is not supported");
+    if (ncomp < 1 || ncomp > 6) return fail(DEMONS_E_ARG, "ncomp must be 1..6");
+    if (!(sigma > 0.f) || !std::isfinite(sigma)) return fail(DEMONS_E_ARG, "sigma must be positive");
+    SmoothArgs sa{};
+    sa.R = gaussian_taps(sigma, sa.w);
+    if (sa.R < 0) return fail(DEMONS_E_UNSUPPORTED, "ceil(3 sigma) exceeds DEMONS_MAX_RADIUS (%d)", DEMONS_MAX_RADIUS);
+    rc = check_ws(c, 1);
+    if (rc != DEMONS_OK) return rc;
+    const Partition p = make_partition(c, 1);
+    sa.d = d;
+    sa.in = d_in;
+    sa.out = d_out;
+    sa.tmp = reinterpret_cast<float*>(c->ws + p.smooth_tmp);
+    sa.ncomp = ncomp;
+    sa.skip = nullptr;
+    sa.force_generic = c->opt_generic_smooth;
+    const int n = launch_smooth(sa, static_cast<cudaStream_t>(stream));
+    if (n < 0) return fail(DEMONS_E_CUDA, "smooth launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    c->launches += n;
+    return DEMONS_OK;
+}
+
+int demons_restrict(demons_ctx* c, const int fine_dims[3], const float* d_fine, float* d_coarse, void* stream) {
+    if (!c) return fail(DEMONS_E_ARG, "ctx is NULL");
+    if (!dims_ok(fine_dims)) return fail(DEMONS_E_ARG, "bad dims");
+    if (!d_fine || !d_coarse) return fail(DEMONS_E_ARG, "NULL volume pointer");
+    const Dims fd{fine_dims[0], fine_dims[1], fine_dims[2]};
+    if (launch_restrict(fd, d_fine, d_coarse, static_cast<cudaStream_t>(stream)) < 0)
+        return fail(DEMONS_E_CUDA, "restrict launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    c->launches += 1;
+    return DEMONS_OK;
+}
+
+int demons_prolong(demons_ctx* c, const int coarse_dims[3], const float* d_uc, const int fine_dims[3], float* d_uf,
+                   void* stream) {
+    if (!c) return fail(DEMONS_E_ARG, "ctx is NULL");
+    if (!dims_ok(coarse_dims) || !dims_ok(fine_dims)) return fail(DEMONS_E_ARG, "bad dims");
+    if (!d_uc || !d_uf) return fail(DEMONS_E_ARG, "NULL field pointer");
+    for (int i = 0; i < 3; ++i)
+        if (coarse_dims[i] != (fine_dims[i] + 1) / 2)
+            return fail(DEMONS_E_ARG, "coarse dims must be ceil(fine dims / 2)");
+    const Dims cd{coarse_dims[0], coarse_dims[1], coarse_dims[2]};
+    const Dims fd{fine_dims[0], fine_dims[1], fine_dims[2]};
+    if (launch_prolong(cd, d_uc, fd, d_uf, static_cast<cudaStream_t>(stream)) < 0)
+        return fail(DEMONS_E_CUDA, "prolong launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    c->launches += 1;
+    return DEMONS_OK;
+}
+
+int demons_ssd(demons_ctx* c, const int dims[3], const float* d_static, const float* d_moving, const float* d_u,
+               const float* d_ub, double* d_out, void* stream) {
+    if (!c) return fail(DEMONS_E_ARG, "ctx is NULL");
+    Dims d;
+    int rc = check_call_dims(c, dims, &d);
+    if (rc != DEMONS_OK) return rc;
+    if (!d_static || !d_moving || !d_u || !d_out) return fail(DEMONS_E_ARG, "NULL pointer");
+    if (is_ic(c) != (d_ub != nullptr)) return fail(DEMONS_E_ARG, "ub must be given exactly for variant 5");
+    rc = check_ws(c, 1);
+    if (rc != DEMONS_OK) return rc;
+    const Partition p = make_partition(c, 1);
+    ReduceScratch rs{reinterpret_cast<double*>(c->ws + p.partials),
+                     &reinterpret_cast<Control*>(c->ws + p.control)->ticket, p.partial_stride};
+    if (launch_ssd(d, d_static, d_moving, d_u, d_ub, d_out, rs, static_cast<cudaStream_t>(stream)) < 0)
+        return fail(DEMONS_E_CUDA, "ssd launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    c->launches += 1;
+    return DEMONS_OK;
+}
+
+int demons_ic_error(demons_ctx* c, const int dims[3], const float* d_uf, const float* d_ub, double* d_out,
+                    void* stream) {
+    if (!c) return fail(DEMONS_E_ARG, "ctx is NULL");
+    Dims d;
+    int rc = check_call_dims(c, dims, &d);
+    if (rc != DEMONS_OK) return rc;
+    if (!d_uf || !d_ub || !d_out) return fail(DEMONS_E_ARG, "NULL pointer");
+    rc = check_ws(c, 1);
+    if (rc != DEMONS_OK) return rc;
+    const Partition p = make_partition(c, 1);
+    ReduceScratch rs{reinterpret_cast<double*>(c->ws + p.partials),
+                     &reinterpret_cast<Control*>(c->ws + p.control)->ticket, p.partial_stride};
+    if (launch_ic_error(d, d_uf, d_ub, d_out, rs, static_cast<cudaStream_t>(stream)) < 0)
+        return fail(DEMONS_E_CUDA, "ic_error launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    c->launches += 1;
+    return DEMONS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,57 @@
+// Host-side launchers of the demons kernels.  Internal to the library (not part of the C ABI).
+#pragma once
+
+#include "common.cuh"
+
+namespace demons {
+
+struct ForceArgs {
+    Dims d;
+    int variant;
+    float alpha2;        // alpha^2 (variant 4; 1 for variant 3)
+    const float* S;      // static image of the level
+    const float* M;      // moving image of the level
+    const float* u_in;   // [3][N]
+    float* u_out;        // [3][N], u_in - F
+    const float* ub_in;  // variant 5
+    float* ub_out;       // variant 5
+    float* Mw;           // workspace, [N]: warped moving image (variants 2-5)
+    float* Sw;           // workspace, [N]: warped static image (variant 5)
+    MetricSink sink;
+    cudaTextureObject_t texM;  // 0 = software trilinear (default)
+    cudaEvent_t ev_mid;        // nullable: recorded between the warp and the force kernel (profiling)
+};
+
+// S1-S4 (+S6).  Returns the number of kernels launched, or -1 with cudaGetLastError() set.
+int launch_warp_force(const ForceArgs& a, cudaStream_t stream);
+
+// Number of per-block partial slots launch_warp_force may use for dims d.
+int force_partial_blocks(const Dims& d);
+
+struct SmoothArgs {
+    Dims d;
+    const float* in;   // [ncomp][N]
+    float* out;        // [ncomp][N]
+    float* tmp;        // workspace [N] (separable fallback only)
+    int ncomp;
+    int R;             // radius
+    float w[33];       // w[k], k = 0..R
+    const int* skip;   // nullable device flag: non-zero = do nothing
+    int force_generic; // 1 = always use the three separable passes
+};
+int launch_smooth(const SmoothArgs& a, cudaStream_t stream);
+
+int launch_restrict(const Dims& fine, const float* in, float* out, cudaStream_t stream);
+int launch_prolong(const Dims& coarse, const float* uc, const Dims& fine, float* uf, cudaStream_t stream);
+
+struct ReduceScratch {
+    double* partials;
+    unsigned int* ticket;
+    int stride;
+};
+int launch_ssd(const Dims& d, const float* S, const float* M, const float* u, const float* ub,
+               double* out, const ReduceScratch& rs, cudaStream_t stream);
+int launch_ic_error(const Dims& d, const float* uf, const float* ub, double* out,
+                    const ReduceScratch& rs, cudaStream_t stream);
+
+}  // namespace demons

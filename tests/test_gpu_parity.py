@@ -1,0 +1,350 @@
+"""GPU parity: every C-ABI entry point against the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): per-kernel outputs |a - b| <= 1e-4 + 1e-5 |b| in fp32;
+final displacement of a full registration within 1e-2 voxel max-abs.  Reductions (fp32 terms,
+fp64 accumulation on both sides): 1e-5 relative.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+VARIANTS = [0, 1, 2, 3, 4, 5]
+ALPHA = {4: 0.4}
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def B(torch_cuda):
+    from paper_0909_0928_b200 import build
+    build.build()
+    from paper_0909_0928_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def P():
+    from paper_0909_0928_b200 import phantoms
+    return phantoms
+
+
+def dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
+
+
+def assert_close(gpu, ref, what, atol=1e-4, rtol=1e-5):
+    gpu = np.asarray(gpu, dtype=np.float64)
+    ref = np.asarray(ref, dtype=np.float64)
+    err = np.abs(gpu - ref) - (atol + rtol * np.abs(ref))
+    worst = np.unravel_index(np.argmax(err), err.shape)
+    assert err.max() <= 0, (f"{what}: max violation {err.max():.3e} at {worst}: gpu {gpu[worst]!r} "
+                            f"ref {ref[worst]!r}")
+
+
+def make_case(P, dims, seed, max_u=3.0):
+    """Blob pair + a smooth non-zero field (+ a second one for the backward field)."""
+    rng = np.random.default_rng(seed)
+    S = P.blob_volume(dims, rng, 20, 10.0)
+    d = P.bump_field(dims, rng, 4, (4.0, 10.0), max_u)
+    M = P.resample(S, d)
+    u = P.bump_field(dims, rng, 6, (3.0, 9.0), max_u, centre_frac=1.0)
+    ub = P.bump_field(dims, rng, 6, (3.0, 9.0), max_u, centre_frac=1.0)
+    return S, M, u, ub
+
+
+# several tiles + ragged tails; (37, 29, 19) and (66, 35, 9) take the scalar (nx % 4 != 0) kernels
+KERNEL_DIMS = [(64, 64, 32), (136, 44, 21), (37, 29, 19), (66, 35, 9), (4, 3, 2), (1, 1, 1)]
+
+
+@pytest.mark.parametrize("dims", KERNEL_DIMS)
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_warp_force_matches_oracle(torch_cuda, B, P, oracle, variant, dims):
+    torch = torch_cuda
+    S, M, u, ub = make_case(P, dims, seed=11 + variant, max_u=min(3.0, max(dims) / 4))
+    alpha = ALPHA.get(variant, 1.0)
+    ic = variant == 5
+    ref_u, ref_ub, ref_m = oracle.warp_force(variant, alpha, S, M, u, ub if ic else None)
+    eng = B.Demons(dims, variant=variant, alpha=alpha)
+    dS, dM, du = dev(torch, S), dev(torch, M), dev(torch, u)
+    dub = dev(torch, ub) if ic else None
+    out = torch.full_like(du, float("nan"))
+    outb = torch.full_like(du, float("nan")) if ic else None
+    met = torch.zeros(3, dtype=torch.float64, device="cuda:0")
+    B.demons_warp_force(eng.ctx, dims, dS, dM, du, out, dub, outb, met)
+    torch.cuda.synchronize()
+    assert_close(out.cpu().numpy(), ref_u, f"u_out variant {variant} dims {dims}")
+    if ic:
+        assert_close(outb.cpu().numpy(), ref_ub, f"ub_out dims {dims}")
+    np.testing.assert_allclose(met.cpu().numpy(), ref_m, rtol=1e-5, atol=1e-6)
+    # metrics are optional and deterministic
+    out2 = torch.empty_like(du)
+    B.demons_warp_force(eng.ctx, dims, dS, dM, du, out2, dub, torch.empty_like(du) if ic else None, None)
+    met2 = torch.zeros(3, dtype=torch.float64, device="cuda:0")
+    B.demons_warp_force(eng.ctx, dims, dS, dM, du, out2, dub, torch.empty_like(du) if ic else None, met2)
+    torch.cuda.synchronize()
+    assert torch.equal(out, out2)
+    assert torch.equal(met, met2), "metrics must be bitwise reproducible"
+    eng.close()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_warp_force_large_displacements_clamp(torch_cuda, B, P, oracle, variant):
+    """Displacements that leave the volume on every side (clamp-to-edge, reading A11)."""
+    torch = torch_cuda
+    dims = (40, 24, 12)
+    S, M, u, ub = make_case(P, dims, seed=5, max_u=30.0)
+    ic = variant == 5
+    alpha = ALPHA.get(variant, 1.0)
+    ref_u, ref_ub, ref_m = oracle.warp_force(variant, alpha, S, M, u, ub if ic else None)
+    eng = B.Demons(dims, variant=variant, alpha=alpha)
+    du = dev(torch, u)
+    out = torch.empty_like(du)
+    outb = torch.empty_like(du) if ic else None
+    met = torch.zeros(3, dtype=torch.float64, device="cuda:0")
+    B.demons_warp_force(eng.ctx, dims, dev(torch, S), dev(torch, M), du, out, dev(torch, ub) if ic else None, outb, met)
+    torch.cuda.synchronize()
+    assert_close(out.cpu().numpy(), ref_u, f"u_out variant {variant}")
+    np.testing.assert_allclose(met.cpu().numpy(), ref_m, rtol=1e-5)
+    eng.close()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_identical_volumes_zero_force(torch_cuda, B, P, variant):  # P1 on the GPU
+    torch = torch_cuda
+    dims = (32, 20, 12)
+    S = P.blob_volume(dims, np.random.default_rng(3), 10, 5.0)
+    eng = B.Demons(dims, variant=variant)
+    dS = dev(torch, S)
+    du = torch.zeros((3,) + S.shape, dtype=torch.float32, device="cuda:0")
+    out = torch.full_like(du, 7.0)
+    ic = variant == 5
+    outb = torch.full_like(du, 7.0) if ic else None
+    met = torch.ones(3, dtype=torch.float64, device="cuda:0")
+    B.demons_warp_force(eng.ctx, dims, dS, dS.clone(), du, out, du.clone() if ic else None, outb, met)
+    torch.cuda.synchronize()
+    assert torch.count_nonzero(out) == 0
+    assert met.cpu().tolist() == [0.0, 0.0, 0.0]
+    eng.close()
+
+
+SMOOTH_DIMS = [(64, 64, 32), (136, 44, 21), (37, 29, 19), (8, 5, 3), (4, 2, 1), (1, 1, 1), (260, 70, 40)]
+
+
+@pytest.mark.parametrize("dims", SMOOTH_DIMS)
+@pytest.mark.parametrize("sigma,ncomp", [(1.0, 3), (2.0, 3), (0.7, 1), (0.3, 2), (3.5, 3), (1.0, 6)])
+def test_smooth_matches_oracle(torch_cuda, B, oracle, dims, sigma, ncomp):
+    torch = torch_cuda
+    rng = np.random.default_rng(17)
+    f = (rng.standard_normal((ncomp, dims[2], dims[1], dims[0])) * 4.0).astype(np.float32)
+    ref = oracle.smooth(f, sigma)
+    eng = B.Demons(dims, variant=5)
+    din = dev(torch, f)
+    out = torch.full_like(din, float("nan"))
+    B.demons_smooth(eng.ctx, dims, din, out, ncomp, sigma)
+    torch.cuda.synchronize()
+    assert_close(out.cpu().numpy(), ref, f"smooth sigma {sigma} dims {dims}")
+    # the separable fallback gives the same answer
+    B.demons_set_option(eng.ctx, "generic_smooth", 1)
+    out2 = torch.full_like(din, float("nan"))
+    B.demons_smooth(eng.ctx, dims, din, out2, ncomp, sigma)
+    torch.cuda.synchronize()
+    assert_close(out2.cpu().numpy(), ref, f"generic smooth sigma {sigma} dims {dims}")
+    eng.close()
+
+
+def test_smooth_preserves_constants(torch_cuda, B):  # P3 on the GPU
+    torch = torch_cuda
+    dims = (72, 40, 24)
+    eng = B.Demons(dims)
+    din = torch.full((3, dims[2], dims[1], dims[0]), 3.25, dtype=torch.float32, device="cuda:0")
+    out = torch.empty_like(din)
+    for sigma in (1.0, 2.0):
+        B.demons_smooth(eng.ctx, dims, din, out, 3, sigma)
+        torch.cuda.synchronize()
+        assert float((out - 3.25).abs().max()) <= 2 * 3.25 * 2 ** -23
+    eng.close()
+
+
+@pytest.mark.parametrize("dims", [(64, 64, 32), (37, 29, 19), (11, 10, 8), (2, 1, 1), (1, 1, 1), (255, 33, 7)])
+def test_restrict_prolong_match_oracle(torch_cuda, B, oracle, dims):
+    torch = torch_cuda
+    rng = np.random.default_rng(23)
+    vol = (rng.standard_normal((dims[2], dims[1], dims[0])) * 100).astype(np.float32)
+    ref = oracle.restrict(vol)
+    eng = B.Demons(dims)
+    cdims = B.demons_level_dims(eng.ctx, 1)
+    assert ref.shape == (cdims[2], cdims[1], cdims[0])
+    out = torch.full(ref.shape, float("nan"), dtype=torch.float32, device="cuda:0")
+    B.demons_restrict(eng.ctx, dims, dev(torch, vol), out)
+    uc = (rng.standard_normal((3,) + ref.shape) * 3).astype(np.float32)
+    ref_f = oracle.prolong(uc, vol.shape)
+    outf = torch.full((3,) + vol.shape, float("nan"), dtype=torch.float32, device="cuda:0")
+    B.demons_prolong(eng.ctx, cdims, dev(torch, uc), dims, outf)
+    torch.cuda.synchronize()
+    assert_close(out.cpu().numpy(), ref, f"restrict {dims}")
+    assert_close(outf.cpu().numpy(), ref_f, f"prolong {dims}")
+    eng.close()
+
+
+@pytest.mark.parametrize("variant", [0, 5])
+def test_ssd_and_ic_error_match_oracle(torch_cuda, B, P, oracle, variant):
+    torch = torch_cuda
+    dims = (44, 36, 22)
+    S, M, u, ub = make_case(P, dims, seed=31)
+    ic = variant == 5
+    eng = B.Demons(dims, variant=variant)
+    out = torch.zeros(2, dtype=torch.float64, device="cuda:0")
+    B.demons_ssd(eng.ctx, dims, dev(torch, S), dev(torch, M), dev(torch, u), dev(torch, ub) if ic else None, out)
+    torch.cuda.synchronize()
+    ref = oracle.final_ssd(variant, S, M, u, ub if ic else None)
+    assert abs(float(out[0]) - ref) <= 1e-5 * ref
+    if ic:
+        B.demons_ic_error(eng.ctx, dims, dev(torch, u), dev(torch, ub), out)
+        torch.cuda.synchronize()
+        mean, mx = oracle.ic_error(u, ub)
+        assert abs(float(out[0]) - mean) <= 1e-5 * mean + 1e-6
+        assert abs(float(out[1]) - mx) <= 1e-5 * mx + 1e-5
+    eng.close()
+
+
+def run_register(torch, B, variant, S, M, iters, alpha=1.0, sigma=1.0, eps=0.0, u0=None, host=False, graphs=True,
+                 stream=True):
+    dims = (S.shape[2], S.shape[1], S.shape[0])
+    ic = variant == 5
+    eng = B.Demons(dims, variant=variant, alpha=alpha, sigma=sigma, levels=len(iters))
+    B.demons_set_option(eng.ctx, "graphs", int(graphs))
+    stats = np.zeros((int(sum(iters)), 3), dtype=np.float64)
+    done = np.zeros(len(iters), dtype=np.int32)
+    st = torch.cuda.Stream() if stream else None
+    if host:
+        hu = np.zeros((3,) + S.shape, np.float32) if u0 is None else u0.copy()
+        hub = np.zeros_like(hu) if ic else None
+        B.demons_register_host(eng.ctx, S, M, hu, hub, iters, eps, stats, done, st)
+        res = dict(u=hu, ub=hub)
+    else:
+        du = torch.zeros((3,) + S.shape, dtype=torch.float32, device="cuda:0") if u0 is None else dev(torch, u0)
+        dub = torch.zeros_like(du) if ic else None
+        dS, dM = dev(torch, S), dev(torch, M)
+        torch.cuda.synchronize()
+        B.demons_register(eng.ctx, dS, dM, du, dub, iters, eps, stats, done, st)
+        torch.cuda.synchronize()
+        res = dict(u=du.cpu().numpy(), ub=dub.cpu().numpy() if ic else None)
+    res.update(stats=stats, iters_done=done.tolist(), launches=B.demons_launch_count(eng.ctx))
+    eng.close()
+    return res
+
+
+def check_registration(res, ref, what):
+    du = np.abs(res["u"] - ref["u"]).max()
+    assert du <= 1e-2, f"{what}: final displacement differs by {du:.3e} voxel"
+    if ref["ub"] is not None:
+        assert np.abs(res["ub"] - ref["ub"]).max() <= 1e-2
+    assert res["iters_done"] == ref["iters_done"], what
+    n = int(sum(ref["iters_done"]))
+    np.testing.assert_allclose(res["stats"][:n], ref["stats"][:n], rtol=2e-4, atol=1e-6, err_msg=what)
+    return du
+
+
+def test_register_config1(torch_cuda, B, P, oracle):
+    """BASELINE.json config 1: 64x64x32 passive, 50 iterations, sigma 1, zero start."""
+    S, M, _ = P.config1_pair()
+    ref = oracle.register(0, 1.0, 1.0, S, M, [50])
+    for kw in (dict(), dict(graphs=False), dict(stream=False), dict(host=True)):
+        res = run_register(torch_cuda, B, 0, S, M, [50], **kw)
+        du = check_registration(res, ref, f"config 1 {kw}")
+        assert res["launches"] > 0
+    assert du < 1e-3  # in practice far inside the 1e-2 bar (tolerance derivation)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_register_all_variants_multilevel(torch_cuda, B, P, oracle, variant):
+    """Three levels with odd sizes (44x36x22 -> 22x18x11 -> 11x9x6), all six variants."""
+    dims = (44, 36, 22)
+    S, M, _ = P.config1_pair(dims=dims, seed=77, max_norm=2.5)
+    alpha = ALPHA.get(variant, 1.0)
+    iters = [12, 10, 8]
+    ref = oracle.register(variant, alpha, 1.0, S, M, iters)
+    res = run_register(torch_cuda, B, variant, S, M, iters, alpha=alpha)
+    check_registration(res, ref, f"variant {variant} 3 levels")
+    res_h = run_register(torch_cuda, B, variant, S, M, iters, alpha=alpha, host=True)
+    assert np.array_equal(res_h["u"], res["u"])
+    if variant == 5:  # P10: from a zero start the two fields are exact negatives
+        assert np.array_equal(res["ub"], -res["u"])
+
+
+def test_register_initial_field_and_sigma2(torch_cuda, B, P, oracle):
+    dims = (40, 32, 20)
+    S, M, u0, _ = make_case(P, dims, seed=41, max_u=1.0)
+    ref = oracle.register(3, 1.0, 2.0, S, M, [9], u0=u0)
+    res = run_register(torch_cuda, B, 3, S, M, [9], sigma=2.0, u0=u0)
+    check_registration(res, ref, "double force, sigma 2, initial field")
+
+
+def test_register_stopping_rule_on_device(torch_cuda, B, P, oracle):
+    """stop when |l_n - l_{n-10}| <= eps; decided on the device, same iteration as
+    the oracle (eps chosen with a wide margin on both sides of the decision)."""
+    dims = (32, 32, 16)
+    S, M, _ = P.config1_pair(dims=dims, seed=9, noise_sd=0.0, max_norm=1.5)
+    iters = [60]
+    full = oracle.register(0, 1.0, 1.0, S, M, iters)
+    st = full["stats"]
+    l = st[1:, 1] / st[1:, 2]                 # l_n, n = 1..59 (l_0 is undefined: U_0 = 0)
+    diff = np.abs(l[10:] - l[:-10])           # n = 11..59
+    best = None
+    for eps in np.sqrt(diff[:-1] * diff[1:]):
+        hit = np.nonzero(diff <= eps)[0]
+        if len(hit) == 0 or not (2 <= hit[0] <= len(diff) - 5):
+            continue
+        k = hit[0]
+        margin = min((diff[:k].min() - eps) / eps, (eps - diff[k]) / eps)
+        if best is None or margin > best[0]:
+            best = (margin, float(eps), 11 + k)
+    assert best is not None and best[0] > 1e-2, "test setup: no eps with a safe margin"
+    eps = best[1]
+    ref = oracle.register(0, 1.0, 1.0, S, M, iters, eps=eps)
+    assert ref["iters_done"] == [best[2] + 1] and 12 < ref["iters_done"][0] < 60
+    for graphs in (True, False):
+        res = run_register(torch_cuda, B, 0, S, M, iters, eps=eps, graphs=graphs)
+        check_registration(res, ref, f"early stop graphs={graphs}")
+        n = int(sum(ref["iters_done"]))
+        assert np.all(res["stats"][n:] == 0.0)
+
+
+def test_alpha_one_equals_double_force_on_gpu(torch_cuda, B, P):  # P8 through the CUDA path
+    dims = (40, 32, 20)
+    S, M, _ = P.config1_pair(dims=dims, seed=13, max_norm=2.0)
+    a = run_register(torch_cuda, B, 3, S, M, [6, 6])
+    b = run_register(torch_cuda, B, 4, S, M, [6, 6], alpha=1.0)
+    assert np.array_equal(a["u"], b["u"])
+
+
+def test_api_rejects_bad_calls(torch_cuda, B):
+    torch = torch_cuda
+    dims = (16, 16, 8)
+    eng = B.Demons(dims, variant=0)
+    f = torch.zeros((3, 8, 16, 16), dtype=torch.float32, device="cuda:0")
+    v = torch.zeros((8, 16, 16), dtype=torch.float32, device="cuda:0")
+    with pytest.raises(B.DemonsError) as e:
+        B.demons_smooth(eng.ctx, dims, f, f, 3, 1.0)  # in place
+    assert e.value.code == B.E_ARG
+    with pytest.raises(B.DemonsError) as e:
+        B.demons_warp_force(eng.ctx, dims, v, v, f, f.clone(), f, None, None)  # ub for a non-IC variant
+    assert e.value.code == B.E_ARG
+    with pytest.raises(B.DemonsError) as e:
+        B.demons_warp_force(eng.ctx, (32, 32, 32), v, v, f, f.clone(), None, None, None)  # larger than ctx
+    assert e.value.code == B.E_WORKSPACE
+    with pytest.raises(B.DemonsError) as e:
+        B.demons_register(eng.ctx, v, v, f, None, [5, 5, 5])  # workspace was sized for one level
+    assert e.value.code == B.E_WORKSPACE
+    with pytest.raises(B.DemonsError) as e:
+        B.demons_smooth(eng.ctx, dims, f, f.clone(), 3, 20.0)
+    assert e.value.code == B.E_UNSUPPORTED
+    eng.close()
