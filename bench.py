@@ -1,0 +1,321 @@
+"""Benchmark of the demons hot path on B200 (contract: one JSON line on stdout from rank 0).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+A "step" is one full registration of BASELINE.json config 2: the 256x256x100 lung-CT-shaped
+phantom pair, passive-force demons (Eq.(1)), single scale, 300 iterations, sigma = 1 -- every
+iteration runs the fused warp+gradient+force+update kernel (with the SSD / relative-norm
+reduction) and the Gaussian smoothing of the field.  `value` is Gvoxel-iterations/s with the
+inputs resident in HBM; `e2e` is the same through demons_register_host with pinned HOST buffers.
+The multi-level variants of configs 3-4 (restrict / prolong included) are timed after the main
+region and reported under "variants".  N > 1: N independent replicas, one process per GPU.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+DIMS = (256, 256, 100)
+SPACING = (0.97, 0.97, 2.5)
+ITERS = [300]
+SIGMA = 1.0
+METRIC = "demons Gvoxel-iter/s (passive force, 256x256x100, 300 iterations, sigma 1; ms_per_step = ms per registration)"
+UNIT = "Gvoxel-iter/s"
+FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
+
+
+def ncu_traffic(kernel_key):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    try:
+        with open(path) as fh:
+            return json.load(fh).get(kernel_key)
+    except Exception:
+        return None
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons while the timed region runs (NVML)."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index = index
+        self.samples = []
+        self.reasons = set()
+        self.max_mhz = None
+        self._halt = threading.Event()
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {
+                nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+                nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake_slowdown",
+                nv.nvmlClocksThrottleReasonApplicationsClocksSetting: "applications_clocks_setting",
+            }
+            while not self._halt.is_set():
+                self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for bit, name in names.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+                time.sleep(0.02)
+        except Exception as e:  # no NVML: report that, do not fail the bench
+            self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
+
+    def stop(self):
+        self._halt.set()
+        self.join(timeout=2)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def physical_gpu_index(local_rank):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+def oracle_sample(S, M, iters):
+    """The oracle as it stands on the host cores: `iters` iterations of the same workload."""
+    from oracle import oracle as O
+    O.build()
+    t0 = time.perf_counter()
+    O.register(0, 1.0, SIGMA, S, M, [iters])
+    return time.perf_counter() - t0
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on a bounded sample of the workload."""
+    from paper_0909_0928_b200 import phantoms, replicas
+    rank, _, world = replicas.env_world()
+    if rank != 0:
+        return
+    S, M, _ = phantoms.lung_pair(DIMS, 202)
+    sample_iters = 2
+    N = DIMS[0] * DIMS[1] * DIMS[2]
+    for _ in range(args.warmup):
+        oracle_sample(S, M, 1)
+    t = 0.0
+    for _ in range(args.steps):
+        t += oracle_sample(S, M, sample_iters)
+    value = args.steps * sample_iters * N / t / 1e9
+    cores = 1
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config2: lung phantom 256x256x100, passive, single scale, sigma 1",
+                   "sample": f"each step = {sample_iters} of the 300 iterations on the full volume pair"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"{args.steps} x {sample_iters} iterations of the 300, full 256x256x100 pair"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def time_registrations(torch, B, eng, dS, dM, du, dub, iters, steps, warmup, stream, replicas):
+    """W untimed + K timed registrations; events on the launching stream; returns seconds."""
+    def one():
+        with torch.cuda.stream(stream):
+            du.zero_()
+            if dub is not None:
+                dub.zero_()
+        B.demons_register(eng.ctx, dS, dM, du, dub, iters, 0.0, None, None, stream)
+
+    for _ in range(warmup):
+        one()
+    torch.cuda.synchronize()
+    replicas.barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = B.demons_launch_count(eng.ctx)
+    ev0.record(stream)
+    for _ in range(steps):
+        one()
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    replicas.barrier()
+    return ev0.elapsed_time(ev1) * 1e-3, B.demons_launch_count(eng.ctx) - l0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-extras", action="store_true", help="skip the per-variant and cpu_baseline legs")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import torch
+    from paper_0909_0928_b200 import binding as B
+    from paper_0909_0928_b200 import build, phantoms, replicas
+
+    build.build()
+    B.lib()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    rank, local_rank, world = replicas.env_world()
+    torch.cuda.set_device(local_rank)
+    device = f"cuda:{local_rank}"
+    replicas.init("nccl")
+    N = DIMS[0] * DIMS[1] * DIMS[2]
+
+    S, M, _ = phantoms.lung_pair(DIMS, replicas.replica_seed(202, rank))
+    dS, dM = torch.from_numpy(S).to(device), torch.from_numpy(M).to(device)
+    du = torch.zeros((3,) + S.shape, dtype=torch.float32, device=device)
+    eng = B.Demons(DIMS, SPACING, B.PASSIVE, 1.0, SIGMA, levels=1, device=device)
+    stream = torch.cuda.Stream(device=device)
+
+    # ---- device-resident timing (the headline `value`) ----
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    sampler.start()
+    secs, launches = time_registrations(torch, B, eng, dS, dM, du, None, ITERS, args.steps, args.warmup, stream,
+                                        replicas)
+    clocks = sampler.stop()
+    units = args.steps * sum(ITERS) * N
+    agg = replicas.aggregate(units, secs, device)
+    final_u_absmax = float(du.abs().max())
+
+    # ---- end to end through the C ABI with pinned host buffers ----
+    hS, hM = torch.from_numpy(S).pin_memory(), torch.from_numpy(M).pin_memory()
+    hu = torch.zeros((3,) + S.shape, dtype=torch.float32).pin_memory()
+    def one_host():
+        hu.zero_()
+        B.demons_register_host(eng.ctx, hS, hM, hu, None, ITERS, 0.0, None, None, stream)
+    for _ in range(2):
+        one_host()
+    torch.cuda.synchronize()
+    replicas.barrier()
+    t0 = time.perf_counter()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    for _ in range(args.steps):
+        one_host()
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    e2e_secs = max(ev0.elapsed_time(ev1) * 1e-3, wall)  # the host-side zeroing of h_u is outside the stream
+    e2e = replicas.aggregate(units, e2e_secs, device)
+    h2d = (2 + 3) * N * 4  # S, M and the initial field (single level: u is an input)
+    d2h = 3 * N * 4
+
+    # ---- per-kernel-class device time inside one more registration ("profile" option) ----
+    B.demons_set_option(eng.ctx, "profile", 1)
+    du.zero_()
+    torch.cuda.synchronize()
+    l0 = B.demons_launch_count(eng.ctx)
+    B.demons_register(eng.ctx, dS, dM, du, None, ITERS, 0.0, None, None, stream)
+    torch.cuda.synchronize()
+    prof = B.demons_get_profile(eng.ctx)
+    launches_per_iter = (B.demons_launch_count(eng.ctx) - l0) / sum(ITERS)
+    B.demons_set_option(eng.ctx, "profile", 0)
+    smooth_launches = launches_per_iter - 1
+    bytes_per_voxel = {"force": 32.0, "smooth": 24.0 if smooth_launches <= 1 else 72.0}
+    kernel_names = {"force": "k_force_fixed<0> (fused warp+gradient+force+update+metrics)",
+                    "smooth": "k_smooth_fused (one pass, 3 components)" if smooth_launches <= 1
+                    else "k_smooth_axis x3 (separable fallback, 3 components)"}
+    peak, peak_src = measured_peak()
+    per_kernel = {}
+    for k in ("force", "smooth"):
+        ms = prof[k]["ms"] / max(prof[k]["groups"], 1)
+        gbs = bytes_per_voxel[k] * N / (ms * 1e-3) / 1e9 if ms > 0 else 0.0
+        per_kernel[k] = {"kernel": kernel_names[k], "avg_ms": ms, "alg_bytes_per_voxel": bytes_per_voxel[k],
+                         "achieved_gbs": gbs, "frac": gbs / peak,
+                         "share_of_step": prof[k]["ms"] / max(prof["force"]["ms"] + prof["smooth"]["ms"], 1e-9)}
+    dom = max(("force", "smooth"), key=lambda k: prof[k]["ms"])
+    roofline = {"bound": "hbm", "kernel": per_kernel[dom]["kernel"], "achieved": per_kernel[dom]["achieved_gbs"],
+                "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": per_kernel[dom]["frac"],
+                "traffic": ncu_traffic(dom), "per_kernel": per_kernel}
+
+    line = {
+        "metric": METRIC, "value": agg["value"] / 1e9, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * agg["seconds"] / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "config2: lung-CT-shaped phantom 256x256x100 fp32, spacing 0.97x0.97x2.5, passive "
+                               "force, single scale, 300 iterations, sigma 1.0",
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": "working set 210 MB (S, M, u, u') > 126 MB L2; no flush between steps",
+                   "graphs": True},
+        "clocks": clocks,
+        "e2e": {"value": e2e["value"] / 1e9, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": 1e3 * e2e["seconds"] / args.steps},
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+        "final_u_absmax_voxel": final_u_absmax,
+    }
+
+    if rank == 0 and world == 1 and not args.no_extras:
+        line["variants"] = bench_variants(torch, B, phantoms, replicas, S, M, device, stream)
+        sample_iters = 6
+        t = oracle_sample(S, M, sample_iters)
+        line["cpu_baseline"] = {"value": sample_iters * N / t / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": f"{sample_iters} of the 300 iterations on the full 256x256x100 pair "
+                                          f"({t:.1f} s, single thread, host has {os.cpu_count()} cores)"}
+    eng.close()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+def bench_variants(torch, B, phantoms, replicas, S, M, device, stream):
+    """BASELINE.json configs 3-4: every variant, three-level pyramid, 100 iterations per level."""
+    out = {}
+    iters = [100, 100, 100]
+    cases = [(0, 1.0, "passive"), (1, 1.0, "evolved_passive"), (2, 1.0, "active"), (3, 1.0, "double"),
+             (4, 0.4, "adjusted_double_a0.4"), (5, 1.0, "inverse_consistent")]
+    dS, dM = torch.from_numpy(S).to(device), torch.from_numpy(M).to(device)
+    for variant, alpha, name in cases:
+        eng = B.Demons(DIMS, SPACING, variant, alpha, SIGMA, levels=3, device=device)
+        du = torch.zeros((3,) + S.shape, dtype=torch.float32, device=device)
+        dub = torch.zeros_like(du) if variant == 5 else None
+        secs, launches = time_registrations(torch, B, eng, dS, dM, du, dub, iters, 3, 2, stream, replicas)
+        voxel_iters = 0
+        for l in range(3):
+            d = B.demons_level_dims(eng.ctx, l)
+            voxel_iters += d[0] * d[1] * d[2] * 100
+        out[name] = {"ms_per_registration": 1e3 * secs / 3, "gvoxel_iter_per_s": 3 * voxel_iters / secs / 1e9,
+                     "launches_per_registration": launches // 3}
+        eng.close()
+    return out
+
+
+if __name__ == "__main__":
+    main()

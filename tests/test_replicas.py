@@ -1,0 +1,52 @@
+"""The N > 1 path (replicas only): world_size-2 gloo processes on CPU."""
+import os
+import socket
+
+import pytest
+import torch.multiprocessing as mp
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _worker(rank, world, port, out):
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port))
+    import torch.distributed as dist
+    from paper_0909_0928_b200 import replicas
+    r, w = replicas.init("gloo")
+    assert (r, w) == (rank, world)
+    replicas.barrier()
+    # rank 1 is the slow one and does more work
+    agg = replicas.aggregate(units_local=10.0 * (rank + 1), seconds_local=1.0 + rank)
+    out.put((rank, agg, replicas.replica_seed(202, rank)))
+    dist.destroy_process_group()
+
+
+def test_aggregate_world_size_2():
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, agg, seed in res:
+        assert agg["units"] == 30.0 and agg["seconds"] == 2.0 and agg["value"] == 15.0
+    assert [s for _, _, s in res] == [202, 1202]
+
+
+def test_single_process_is_identity():
+    from paper_0909_0928_b200 import replicas
+    for k in ("RANK", "LOCAL_RANK", "WORLD_SIZE"):
+        os.environ.pop(k, None)
+    assert replicas.env_world() == (0, 0, 1)
+    assert replicas.aggregate(6.0, 2.0) == {"units": 6.0, "seconds": 2.0, "value": 3.0}
