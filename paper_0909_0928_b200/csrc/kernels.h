@@ -38,6 +38,7 @@ struct SmoothArgs {
     float w[33];       // w[k], k = 0..R
     const int* skip;   // nullable device flag: non-zero = do nothing
     int force_generic; // 1 = always use the three separable passes
+    int zc_override;   // > 0: planes per CTA of the fused kernel (tuning)
 };
 int launch_smooth(const SmoothArgs& a, cudaStream_t stream);
 

@@ -1,0 +1,119 @@
+"""BASELINE.json config 5: bandwidth sweep of the per-iteration kernels through the C ABI.
+
+    python -m paper_0909_0928_b200.sweep [--sizes 128x128x64,256x256x100,...] [--reps 20]
+                                         [--kernels force,smooth,pyramid] [--json out.json]
+
+For every size: the fused warp+force+update entry point for all six variants, the Gaussian
+smoothing at sigma 1.0 and 2.0 (3 components), restrict and prolong.  Inputs are the seeded blob
+phantom and a random smooth field with max |u| = 8 voxels (phantoms.sweep_inputs).  Reported per
+kernel: median CUDA-event time of `reps` launches after 3 warm-ups, effective GB/s = algorithmic
+bytes (DESIGN.md byte table) / time, and % of the measured HBM peak.  The same command with
+--reps 3 is what the ncu captures under profiles/ run.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+SEEDS = {(128, 128, 64): 500, (256, 256, 100): 501, (512, 512, 160): 502, (512, 512, 256): 503}
+# algorithmic bytes per voxel of each entry point as implemented
+FORCE_BYTES = {0: 32.0, 1: 32.0, 2: 52.0, 3: 52.0, 4: 52.0, 5: 96.0}
+VARIANT_NAMES = ["passive", "evolved_passive", "active", "double", "adjusted_double", "inverse_consistent"]
+
+
+def hbm_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured"
+    except Exception:
+        return 6650.0, "fallback"
+
+
+def median_ms(torch, stream, fn, reps):
+    for _ in range(3):
+        fn()
+    torch.cuda.synchronize()
+    times = []
+    for _ in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        fn()
+        e1.record(stream)
+        e1.synchronize()
+        times.append(e0.elapsed_time(e1))
+    return float(np.median(times))
+
+
+def run(sizes, kernels, reps, device="cuda:0"):
+    import torch
+    from . import binding as B
+    from . import build, phantoms
+    build.build()
+    B.lib()
+    peak, peak_kind = hbm_peak()
+    stream = torch.cuda.Stream(device=device)
+    rows = []
+    for dims in sizes:
+        N = dims[0] * dims[1] * dims[2]
+        S, M, u = phantoms.sweep_inputs(dims, SEEDS.get(tuple(dims), 599))
+        dS, dM, du = (torch.from_numpy(a).to(device) for a in (S, M, u))
+        dub = (-du).contiguous()
+        out, outb = torch.empty_like(du), torch.empty_like(du)
+        met = torch.zeros(3, dtype=torch.float64, device=device)
+
+        def add(name, ms, nbytes):
+            gbs = nbytes / (ms * 1e-3) / 1e9
+            rows.append({"dims": "x".join(map(str, dims)), "kernel": name, "ms": ms, "alg_bytes": nbytes,
+                         "gbs": gbs, "pct_of_peak": 100.0 * gbs / peak})
+
+        if "force" in kernels:
+            for variant in range(6):
+                eng = B.Demons(dims, variant=variant, alpha=0.4 if variant == 4 else 1.0, device=device)
+                ic = variant == 5
+                ms = median_ms(torch, stream, lambda: B.demons_warp_force(
+                    eng.ctx, dims, dS, dM, du, out, dub if ic else None, outb if ic else None, met, stream), reps)
+                add(f"warp_force[{VARIANT_NAMES[variant]}]", ms, FORCE_BYTES[variant] * N)
+                eng.close()
+        eng = B.Demons(dims, variant=0, device=device)
+        if "smooth" in kernels:
+            for sigma in (1.0, 2.0):
+                ms = median_ms(torch, stream, lambda: B.demons_smooth(eng.ctx, dims, du, out, 3, sigma, stream), reps)
+                add(f"smooth[sigma={sigma}]", ms, 24.0 * N)
+        if "pyramid" in kernels:
+            cd = B.demons_level_dims(eng.ctx, 1)
+            coarse = torch.empty((cd[2], cd[1], cd[0]), dtype=torch.float32, device=device)
+            uc = torch.randn((3, cd[2], cd[1], cd[0]), dtype=torch.float32, device=device)
+            ms = median_ms(torch, stream, lambda: B.demons_restrict(eng.ctx, dims, dS, coarse, stream), reps)
+            add("restrict", ms, 4.5 * N)
+            ms = median_ms(torch, stream, lambda: B.demons_prolong(eng.ctx, cd, uc, dims, out, stream), reps)
+            add("prolong", ms, 13.5 * N)
+        eng.close()
+    return rows, peak, peak_kind
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--sizes", default="128x128x64,256x256x100,512x512x160,512x512x256")
+    ap.add_argument("--kernels", default="force,smooth,pyramid")
+    ap.add_argument("--reps", type=int, default=20)
+    ap.add_argument("--json", default=None)
+    args = ap.parse_args()
+    sizes = [tuple(int(v) for v in s.split("x")) for s in args.sizes.split(",")]
+    rows, peak, kind = run(sizes, set(args.kernels.split(",")), args.reps)
+    print(f"# HBM peak {peak:.1f} GB/s ({kind}); effective GB/s = algorithmic bytes / median time")
+    print(f"{'dims':>12} {'kernel':<34} {'ms':>9} {'GB/s':>9} {'% peak':>7}")
+    for r in rows:
+        print(f"{r['dims']:>12} {r['kernel']:<34} {r['ms']:9.4f} {r['gbs']:9.1f} {r['pct_of_peak']:7.1f}")
+    if args.json:
+        with open(args.json, "w") as fh:
+            json.dump({"peak_gbs": peak, "peak_kind": kind, "rows": rows}, fh, indent=1)
+
+
+if __name__ == "__main__":
+    sys.path.insert(0, ROOT)
+    main()
