@@ -9,6 +9,7 @@
 
 namespace demons {
 
+int launch_smooth_tma(const SmoothArgs& a, cudaStream_t st);    // smooth_tma.cu; 0 = not applicable
 int launch_smooth_fused(const SmoothArgs& a, cudaStream_t st);  // smooth_fused.cu; 0 = not applicable
 
 namespace {
@@ -49,7 +50,9 @@ __global__ void __launch_bounds__(256) k_smooth_axis(const float* __restrict__ i
 
 int launch_smooth(const SmoothArgs& a, cudaStream_t st) {
     if (!a.force_generic) {
-        const int n = launch_smooth_fused(a, st);
+        int n = a.no_tma ? 0 : launch_smooth_tma(a, st);
+        if (n != 0) return n;
+        n = launch_smooth_fused(a, st);
         if (n != 0) return n;
     }
     Taps t;

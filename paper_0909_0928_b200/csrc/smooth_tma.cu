@@ -1,0 +1,347 @@
+// S5, B200 fast path: the whole separable Gaussian (reading A9) in ONE pass
+// over the field, fed by TMA.
+//
+// A CTA owns a 128-wide (x) by TY-high (y) tile and marches along z.  Per plane:
+//   * one elected thread issues a 4D `cp.async.bulk.tensor` (TMA) load of the tile plus its
+//     y/x halo into a STAGES-deep shared-memory ring, completion on an mbarrier -- no load
+//     instructions, no address arithmetic, no registers spent on prefetch;
+//   * y pass in registers from shared memory (a thread owns one float4 column of K rows and reads
+//     the K + 2R rows it needs), packed f32x2 arithmetic (FFMA2 / FADD2 on sm_100);
+//   * x pass through a small shared-memory exchange of the y-smoothed float4s; the halo columns
+//     of the tile are y-smoothed by a few lanes of one extra warp (which also issues the TMA);
+//   * z pass in registers: a ring of the last 2R + 1 xy-smoothed planes, statically indexed by
+//     unrolling the march by the ring length; 128-bit coalesced stores.
+// Borders replicate the edge value (index clamp) on every axis, exactly as the oracle's clamp:
+// TMA zero-fills outside the volume, and those cells are never read -- rows / column groups are
+// clamped when the shared-memory addresses are formed.
+// HBM sees every element once in and once out (8 B / element); the paper's design was one
+// kernel per axis through shared memory (L175), i.e. 24 B / element.
+#include <cuda.h>
+
+#include "kernels.h"
+
+namespace demons {
+
+namespace {
+
+struct Taps {
+    float w[8];
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2,
+                                            int c3) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+        : "memory");
+}
+
+struct F4 {  // a float4 as two packed pairs
+    float2 a, b;
+};
+__device__ __forceinline__ F4 ld_f4(const float* p) {
+    const float4 q = *reinterpret_cast<const float4*>(p);
+    F4 r;
+    r.a = make_float2(q.x, q.y);
+    r.b = make_float2(q.z, q.w);
+    return r;
+}
+
+template <int R, int K, int RG, int STAGES>
+struct Cfg {
+    static constexpr int NH = (R + 3) / 4;      // halo float4 groups per side
+    static constexpr int L = 2 * R + 1;         // ring length
+    static constexpr int GX = 32;               // owner float4 groups per row (one warp wide)
+    static constexpr int GW = GX + 2 * NH;      // groups per shared row
+    static constexpr int TY = RG * K;           // output rows per tile
+    static constexpr int ROWS = TY + 2 * R;     // rows per loaded plane
+    static constexpr int BOXW = 4 * GW;         // floats per loaded row
+    static constexpr int STAGE_BYTES = (ROWS * BOXW * 4 + 127) / 128 * 128;
+    static constexpr int XS_BYTES = 2 * TY * GW * 16;
+    static constexpr int THREADS = 32 * (RG + 1);
+    static constexpr int SMEM = STAGES * STAGE_BYTES + XS_BYTES + STAGES * 8 + 128;
+    static_assert(2 * NH * RG <= 32, "halo jobs must fit one warp");
+    static_assert(TY >= R, "tile must be at least R rows high");
+};
+
+template <int R, int K, int RG, int STAGES>
+__global__ void __launch_bounds__(32 * (RG + 1))
+    k_smooth_tma(const __grid_constant__ CUtensorMap tmap, float* __restrict__ out, const Dims d, const int zc,
+                 const int tiles_x, const Taps t, const int* __restrict__ skip) {
+    using C = Cfg<R, K, RG, STAGES>;
+    constexpr int NH = C::NH, L = C::L, GX = C::GX, GW = C::GW, TY = C::TY, BOXW = C::BOXW;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    float4* xs = reinterpret_cast<float4*>(smem + STAGES * C::STAGE_BYTES);  // [2][TY][GW]
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem + STAGES * C::STAGE_BYTES + C::XS_BYTES);
+
+    if (skip != nullptr && *reinterpret_cast<const volatile int*>(skip) != 0) return;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const bool halo_warp = warp == RG;
+    const int tile_x = blockIdx.x % tiles_x, tile_y = blockIdx.x / tiles_x;
+    const int x0 = tile_x * GX * 4, y0 = tile_y * TY;
+    const int comp = blockIdx.z;
+    const int z_start = blockIdx.y * zc;
+    const int nplanes = min(zc, d.nz - z_start);
+    const int P = nplanes + 2 * R;
+    const size_t plane = (size_t)d.nx * d.ny;
+
+    // role of this thread: which float4 group (g) of which row group (rg)
+    int g, rg;
+    bool active;
+    if (!halo_warp) {
+        g = lane + NH;
+        rg = warp;
+        active = true;
+    } else {
+        rg = lane / (2 * NH);
+        const int h = lane % (2 * NH);
+        g = h < NH ? h : GX + h;  // left groups 0..NH-1, right groups GX+NH..GW-1
+        active = lane < 2 * NH * RG;
+        if (!active) rg = 0;
+    }
+    const int xg = x0 + 4 * (g - NH);
+    const int xg_c = min(max(xg, 0), d.nx - 4);
+    const int gc = (xg_c - (x0 - 4 * NH)) >> 2;  // group actually read (clamp = replicate)
+    const bool owner = !halo_warp && xg < d.nx;
+    const bool outside = xg < 0 || xg >= d.nx;
+    int rowoff[K + 2 * R];
+#pragma unroll
+    for (int i = 0; i < K + 2 * R; ++i) {
+        const int y = min(max(y0 + rg * K - R + i, 0), d.ny - 1);
+        rowoff[i] = (y - (y0 - R)) * BOXW + 4 * gc;
+    }
+    float2 w2[R + 1];
+#pragma unroll
+    for (int k = 0; k <= R; ++k) w2[k] = make_float2(t.w[k], t.w[k]);
+
+    const bool issuer = halo_warp && lane == 0;
+    auto issue = [&](int p) {  // plane p of the march -> stage p % STAGES
+        const int s = p % STAGES;
+        const int z = min(max(z_start - R + p, 0), d.nz - 1);
+        mbar_expect_tx(&full[s], (uint32_t)(C::ROWS * BOXW * 4));
+        tma_load_4d(smem + s * C::STAGE_BYTES, &tmap, &full[s], x0 - 4 * NH, y0 - R, z, comp);
+    };
+    if (issuer) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+    if (issuer) {
+        for (int p = 0; p < STAGES && p < P; ++p) issue(p);
+    }
+
+    float* dst = out + (size_t)comp * plane * d.nz + (size_t)(y0 + rg * K) * d.nx + xg;
+    F4 ring[L][K];
+    for (int pg = 0; pg < P; pg += L) {
+#pragma unroll
+        for (int s = 0; s < L; ++s) {
+            const int p = pg + s;
+            if (p < P) {  // uniform over the CTA
+                const int stage = p % STAGES;
+                mbar_wait(&full[stage], (uint32_t)((p / STAGES) & 1));
+                const float* raw = reinterpret_cast<const float*>(smem + stage * C::STAGE_BYTES);
+                float4* xrow = xs + ((p & 1) * TY + rg * K) * GW;
+                F4 ys[K];
+                if (active) {
+                    // ---- y pass: registers, packed f32x2 ----
+                    F4 v[K + 2 * R];
+#pragma unroll
+                    for (int i = 0; i < K + 2 * R; ++i) v[i] = ld_f4(raw + rowoff[i]);
+#pragma unroll
+                    for (int j = 0; j < K; ++j) {
+                        float2 a = __fmul2_rn(w2[0], v[j + R].a), b = __fmul2_rn(w2[0], v[j + R].b);
+#pragma unroll
+                        for (int k = 1; k <= R; ++k) {
+                            a = __ffma2_rn(w2[k], __fadd2_rn(v[j + R - k].a, v[j + R + k].a), a);
+                            b = __ffma2_rn(w2[k], __fadd2_rn(v[j + R - k].b, v[j + R + k].b), b);
+                        }
+                        if (outside) {  // rare: halo lanes / ragged tiles at the volume border
+                            if (xg < 0) {  // left of the volume: replicate x = 0
+                                a = make_float2(a.x, a.x);
+                                b = a;
+                            } else {  // right of the volume: replicate x = nx - 1
+                                b = make_float2(b.y, b.y);
+                                a = b;
+                            }
+                        }
+                        ys[j].a = a;
+                        ys[j].b = b;
+                        xrow[j * GW + g] = make_float4(a.x, a.y, b.x, b.y);
+                    }
+                }
+                __syncthreads();  // xs complete; every warp is done reading this raw stage
+                if (issuer && p + STAGES < P) issue(p + STAGES);
+                if (owner) {
+                    // ---- x pass: neighbours' float4s from the exchange buffer ----
+#pragma unroll
+                    for (int j = 0; j < K; ++j) {
+                        float a[4 * (2 * NH + 1)];
+#pragma unroll
+                        for (int h = 0; h < 2 * NH + 1; ++h) {
+                            if (h == NH) {
+                                a[4 * h + 0] = ys[j].a.x;
+                                a[4 * h + 1] = ys[j].a.y;
+                                a[4 * h + 2] = ys[j].b.x;
+                                a[4 * h + 3] = ys[j].b.y;
+                            } else {
+                                const float4 q = xrow[j * GW + g - NH + h];
+                                a[4 * h + 0] = q.x;
+                                a[4 * h + 1] = q.y;
+                                a[4 * h + 2] = q.z;
+                                a[4 * h + 3] = q.w;
+                            }
+                        }
+                        float o[4];
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            float acc = t.w[0] * a[4 * NH + e];
+#pragma unroll
+                            for (int k = 1; k <= R; ++k) acc = fmaf(t.w[k], a[4 * NH + e - k] + a[4 * NH + e + k], acc);
+                            o[e] = acc;
+                        }
+                        ring[s][j].a = make_float2(o[0], o[1]);
+                        ring[s][j].b = make_float2(o[2], o[3]);
+                    }
+                    // ---- z pass: register ring, packed f32x2 ----
+                    if (p >= 2 * R) {
+                        float* orow = dst + (size_t)(z_start + p - 2 * R) * plane;
+#pragma unroll
+                        for (int j = 0; j < K; ++j) {
+                            const F4& c = ring[(s - R + L) % L][j];
+                            float2 a = __fmul2_rn(w2[0], c.a), b = __fmul2_rn(w2[0], c.b);
+#pragma unroll
+                            for (int k = 1; k <= R; ++k) {
+                                const F4& lo = ring[(s - R - k + 2 * L) % L][j];
+                                const F4& hi = ring[(s - R + k + L) % L][j];
+                                a = __ffma2_rn(w2[k], __fadd2_rn(lo.a, hi.a), a);
+                                b = __ffma2_rn(w2[k], __fadd2_rn(lo.b, hi.b), b);
+                            }
+                            if (y0 + rg * K + j < d.ny)
+                                *reinterpret_cast<float4*>(orow + (size_t)j * d.nx) = make_float4(a.x, a.y, b.x, b.y);
+                        }
+                    }
+                }
+            }
+        }
+    }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+        else
+            cudaGetLastError();
+    }
+    return fn;
+}
+
+template <int R, int K, int RG, int STAGES>
+int launch_cfg(const SmoothArgs& a, int zc, cudaStream_t st) {
+    using C = Cfg<R, K, RG, STAGES>;
+    EncodeTiledFn enc = encode_fn();
+    if (!enc) return 0;
+    const Dims d = a.d;
+    alignas(64) CUtensorMap map;
+    const cuuint64_t gdim[4] = {(cuuint64_t)d.nx, (cuuint64_t)d.ny, (cuuint64_t)d.nz, (cuuint64_t)a.ncomp};
+    const cuuint64_t gstr[3] = {(cuuint64_t)d.nx * 4, (cuuint64_t)d.nx * d.ny * 4, (cuuint64_t)d.nx * d.ny * d.nz * 4};
+    const cuuint32_t box[4] = {(cuuint32_t)C::BOXW, (cuuint32_t)C::ROWS, 1, 1};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    if (enc(&map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<float*>(a.in), gdim, gstr, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return 0;
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM) !=
+            cudaSuccess) {
+            cudaGetLastError();
+            return 0;
+        }
+        attr_set = true;
+    }
+    const int tiles_x = (d.nx + C::GX * 4 - 1) / (C::GX * 4);
+    const int tiles_y = (d.ny + C::TY - 1) / C::TY;
+    const int chunks = (d.nz + zc - 1) / zc;
+    if (chunks > 65535) return 0;
+    Taps t;
+    for (int k = 0; k < 8; ++k) t.w[k] = k <= a.R ? a.w[k] : 0.f;
+    const dim3 grid(tiles_x * tiles_y, chunks, a.ncomp);
+    k_smooth_tma<R, K, RG, STAGES><<<grid, C::THREADS, C::SMEM, st>>>(map, a.out, d, zc, tiles_x, t, a.skip);
+    return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+}
+
+// Planes per CTA: the number of z chunks that minimises  waves x (planes per chunk + 2R warm-up).
+int pick_zc(const SmoothArgs& a, int tile_w, int tile_h, int slots) {
+    const long long tiles = (long long)((a.d.nx + tile_w - 1) / tile_w) * ((a.d.ny + tile_h - 1) / tile_h) * a.ncomp;
+    int best_zc = a.d.nz;
+    double best = 1e300;
+    for (int chunks = 1; chunks <= a.d.nz; ++chunks) {
+        const int zc = (a.d.nz + chunks - 1) / chunks;
+        if (chunks > 1 && zc < 2 * a.R) break;
+        const long long ctas = tiles * ((a.d.nz + zc - 1) / zc);
+        const double waves = (double)((ctas + slots - 1) / slots);
+        const double cost = waves * (zc + 2 * a.R + 2);
+        if (cost < best - 1e-9) {
+            best = cost;
+            best_zc = zc;
+        }
+    }
+    return best_zc;
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+}  // namespace
+
+// Returns launches (1), 0 if this path does not apply (caller falls back), -1 on a launch error.
+int launch_smooth_tma(const SmoothArgs& a, cudaStream_t st) {
+    if (a.d.nx % 4 != 0 || a.d.nx < 4 || !aligned16(a.in) || !aligned16(a.out)) return 0;
+    if (a.R < 1 || a.R > 6) return 0;
+    const int zc = a.zc_override > 0 ? a.zc_override : pick_zc(a, 128, 16, 148 * 2);
+    switch (a.R) {
+    case 1: return launch_cfg<1, 2, 8, 4>(a, zc, st);
+    case 2: return launch_cfg<2, 2, 8, 4>(a, zc, st);
+    case 3: return launch_cfg<3, 2, 8, 4>(a, zc, st);
+    case 4: return launch_cfg<4, 2, 8, 4>(a, zc, st);
+    case 5: return launch_cfg<5, 2, 8, 3>(a, zc, st);
+    case 6: return launch_cfg<6, 2, 8, 3>(a, zc, st);
+    default: return 0;
+    }
+}
+
+}  // namespace demons
