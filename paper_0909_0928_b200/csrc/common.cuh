@@ -38,28 +38,31 @@ constexpr int LHIST = 16;  // power of two >= 11 (lag of 10 iterations)
 __device__ __forceinline__ float lerpf(float a, float b, float t) { return fmaf(t, b - a, a); }
 
 // One axis of O2 (reading A11): p = x + u clamped to [0, n-1], i0 = floor(p), f = p - i0,
-// i1 = min(i0 + 1, n - 1).  The split is taken on u, not on x + u: floor(x + u) = x + floor(u)
-// for integer x and u - floor(u) is exact in fp32, so no bits of the fraction are lost to the
-// magnitude of x.
+// i1 = min(i0 + 1, n - 1).
+//  * The split is taken on u, not on x + u: floor(x + u) = x + floor(u) for integer x and
+//    u - floor(u) is exact in fp32, so no bits of the fraction are lost to the magnitude of x.
+//  * floor without the conversion unit: for |u| <= 2^21, t = u + 1.5*2^23 has ulp 1, so
+//    t - 1.5*2^23 = rint(u) exactly and the low mantissa bits of t are that integer.
+//  * The clamp is taken on the two indices: when p is outside [0, n-1] both become the same edge
+//    voxel and lerp(a, a, f) = a exactly, which is what clamping p does.
 __device__ __forceinline__ void split_axis(int x, float u, int n, int& i0, int& i1, float& f) {
-    float fl = floorf(u);
-    f = u - fl;
-    fl = fminf(fmaxf(fl, -16777216.f), 16777216.f);
-    int i = x + (int)fl;
-    if (i < 0) {
-        i = 0;
-        f = 0.f;
+    u = fminf(fmaxf(u, -2097152.f), 2097152.f);
+    const float t = u + 12582912.f;
+    float r = t - 12582912.f;
+    int i = __float_as_int(t) - 0x4B400000;
+    if (r > u) {
+        r -= 1.f;
+        i -= 1;
     }
-    if (i >= n - 1) {
-        i = n - 1;
-        f = 0.f;
-    }
-    i0 = i;
-    i1 = min(i + 1, n - 1);
+    f = u - r;
+    i += x;
+    i0 = min(max(i, 0), n - 1);
+    i1 = min(max(i + 1, 0), n - 1);
 }
 
 // Software trilinear sample of I at (x + ux, y + uy, z + uz): PAPER.md L179-181 ("our own
-// trilinear interpolation function").  Interpolates along x, then y, then z.
+// trilinear interpolation function").  Interpolates along x, then y, then z.  32-bit offsets
+// (volumes have fewer than 2^29 voxels, checked by demons_create).
 __device__ __forceinline__ float trilinear(const float* __restrict__ I, const Dims& d, int x, int y,
                                            int z, float ux, float uy, float uz) {
     int x0, x1, y0, y1, z0, z1;
@@ -67,14 +70,13 @@ __device__ __forceinline__ float trilinear(const float* __restrict__ I, const Di
     split_axis(x, ux, d.nx, x0, x1, fx);
     split_axis(y, uy, d.ny, y0, y1, fy);
     split_axis(z, uz, d.nz, z0, z1, fz);
-    const float* p00 = I + ((size_t)z0 * d.ny + y0) * d.nx;
-    const float* p10 = I + ((size_t)z0 * d.ny + y1) * d.nx;
-    const float* p01 = I + ((size_t)z1 * d.ny + y0) * d.nx;
-    const float* p11 = I + ((size_t)z1 * d.ny + y1) * d.nx;
-    const float c000 = __ldg(p00 + x0), c100 = __ldg(p00 + x1);
-    const float c010 = __ldg(p10 + x0), c110 = __ldg(p10 + x1);
-    const float c001 = __ldg(p01 + x0), c101 = __ldg(p01 + x1);
-    const float c011 = __ldg(p11 + x0), c111 = __ldg(p11 + x1);
+    const int zo0 = z0 * d.ny, zo1 = z1 * d.ny;
+    const int r00 = (zo0 + y0) * d.nx, r10 = (zo0 + y1) * d.nx;
+    const int r01 = (zo1 + y0) * d.nx, r11 = (zo1 + y1) * d.nx;
+    const float c000 = __ldg(I + (unsigned)(r00 + x0)), c100 = __ldg(I + (unsigned)(r00 + x1));
+    const float c010 = __ldg(I + (unsigned)(r10 + x0)), c110 = __ldg(I + (unsigned)(r10 + x1));
+    const float c001 = __ldg(I + (unsigned)(r01 + x0)), c101 = __ldg(I + (unsigned)(r01 + x1));
+    const float c011 = __ldg(I + (unsigned)(r11 + x0)), c111 = __ldg(I + (unsigned)(r11 + x1));
     const float a00 = lerpf(c000, c100, fx), a10 = lerpf(c010, c110, fx);
     const float a01 = lerpf(c001, c101, fx), a11 = lerpf(c011, c111, fx);
     const float b0 = lerpf(a00, a10, fy), b1 = lerpf(a01, a11, fy);
@@ -112,16 +114,16 @@ template <int VEC>
 __device__ __forceinline__ void centre_and_gradient(const float* __restrict__ I, const Dims& d, int x0,
                                                     int y, int z, float (&c)[VEC], float (&gx)[VEC],
                                                     float (&gy)[VEC], float (&gz)[VEC]) {
-    const size_t plane = (size_t)d.nx * d.ny;
-    const float* row = I + (size_t)z * plane + (size_t)y * d.nx;
+    const int plane = d.nx * d.ny;
+    const int row = z * plane + y * d.nx;
     float ym[VEC], yp[VEC], zm[VEC], zp[VEC];
-    load_vec<VEC>(row + x0, c);
-    const float xm = __ldg(row + max(x0 - 1, 0));
-    const float xp = __ldg(row + min(x0 + VEC, d.nx - 1));
-    load_vec<VEC>(I + (size_t)z * plane + (size_t)max(y - 1, 0) * d.nx + x0, ym);
-    load_vec<VEC>(I + (size_t)z * plane + (size_t)min(y + 1, d.ny - 1) * d.nx + x0, yp);
-    load_vec<VEC>(I + (size_t)max(z - 1, 0) * plane + (size_t)y * d.nx + x0, zm);
-    load_vec<VEC>(I + (size_t)min(z + 1, d.nz - 1) * plane + (size_t)y * d.nx + x0, zp);
+    load_vec<VEC>(I + (unsigned)(row + x0), c);
+    const float xm = __ldg(I + (unsigned)(row + max(x0 - 1, 0)));
+    const float xp = __ldg(I + (unsigned)(row + min(x0 + VEC, d.nx - 1)));
+    load_vec<VEC>(I + (unsigned)(row + x0 - (y > 0 ? d.nx : 0)), ym);
+    load_vec<VEC>(I + (unsigned)(row + x0 + (y < d.ny - 1 ? d.nx : 0)), yp);
+    load_vec<VEC>(I + (unsigned)(row + x0 - (z > 0 ? plane : 0)), zm);
+    load_vec<VEC>(I + (unsigned)(row + x0 + (z < d.nz - 1 ? plane : 0)), zp);
 #pragma unroll
     for (int j = 0; j < VEC; ++j) {
         const float l = j > 0 ? c[j - 1] : xm;
@@ -130,6 +132,13 @@ __device__ __forceinline__ void centre_and_gradient(const float* __restrict__ I,
         gy[j] = 0.5f * (yp[j] - ym[j]);
         gz[j] = 0.5f * (zp[j] - zm[j]);
     }
+}
+
+// sqrt on the special-function unit (relative error ~2^-22); used for the metrics only.
+__device__ __forceinline__ float fast_sqrt(float x) {
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
 }
 
 // q(num, den) = den > 1e-9 ? num/den : 0 -- the zero guard of reading A6.

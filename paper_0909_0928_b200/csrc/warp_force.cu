@@ -66,6 +66,7 @@ struct KParams {
     float* Sw;
     MetricSink sink;
     cudaTextureObject_t texM;
+    int zper;  // consecutive planes per block
 };
 
 // ---- variants 0, 1: fused warp + gradient + force + update ------------------------------------
@@ -73,14 +74,14 @@ template <int VARIANT, int VEC, bool TEX>
 __global__ void __launch_bounds__(BX* BY) k_force_fixed(const KParams p) {
     if (skip_pass(p.sink)) return;
     const Dims d = p.d;
-    const size_t N = nvox(d);
+    const unsigned N = (unsigned)nvox(d);
     const int x0 = (blockIdx.x * BX + threadIdx.x) * VEC;
     const int y = blockIdx.y * BY + threadIdx.y;
     const bool active = x0 < d.nx && y < d.ny;
     double acc[3] = {0.0, 0.0, 0.0};
     if (active) {
-        for (int z = blockIdx.z; z < d.nz; z += gridDim.z) {
-            const size_t i0 = ((size_t)z * d.ny + y) * d.nx + x0;
+        for (int z = blockIdx.z * p.zper; z < min(d.nz, (int)(blockIdx.z + 1) * p.zper); ++z) {
+            const unsigned i0 = (unsigned)((z * d.ny + y) * d.nx + x0);
             float ux[VEC], uy[VEC], uz[VEC];
             load_vec<VEC>(p.u_in + i0, ux);
             load_vec<VEC>(p.u_in + N + i0, uy);
@@ -109,7 +110,7 @@ __global__ void __launch_bounds__(BX* BY) k_force_fixed(const KParams p) {
                     const float dd = mw[j] - s[j];
                     const float s2 = fmaf(gx[j], gx[j], fmaf(gy[j], gy[j], gz[j] * gz[j]));
                     const float m2 = fmaf(hx[j], hx[j], fmaf(hy[j], hy[j], hz[j] * hz[j]));
-                    const float num = 4.f * dd * sqrtf(s2) * sqrtf(m2);
+                    const float num = 4.f * dd * fast_sqrt(s2) * fast_sqrt(m2);
                     const float den = (fmaf(2.f * dd, dd, s2 + m2)) * (s2 + m2);
                     k[j] = guarded_div(num, den);
                 }
@@ -124,8 +125,8 @@ __global__ void __launch_bounds__(BX* BY) k_force_fixed(const KParams p) {
                 oy[j] = uy[j] - fy;
                 oz[j] = uz[j] - fz;
                 ssd = fmaf(dd, dd, ssd);
-                sf += sqrtf(fmaf(fx, fx, fmaf(fy, fy, fz * fz)));
-                su += sqrtf(fmaf(ux[j], ux[j], fmaf(uy[j], uy[j], uz[j] * uz[j])));
+                sf += fast_sqrt(fmaf(fx, fx, fmaf(fy, fy, fz * fz)));
+                su += fast_sqrt(fmaf(ux[j], ux[j], fmaf(uy[j], uy[j], uz[j] * uz[j])));
             }
             store_vec<VEC>(p.u_out + i0, ox);
             store_vec<VEC>(p.u_out + N + i0, oy);
@@ -146,12 +147,12 @@ template <int VEC, bool IC, bool TEX>
 __global__ void __launch_bounds__(BX* BY) k_warp(const KParams p) {
     if (skip_pass(p.sink)) return;
     const Dims d = p.d;
-    const size_t N = nvox(d);
+    const unsigned N = (unsigned)nvox(d);
     const int x0 = (blockIdx.x * BX + threadIdx.x) * VEC;
     const int y = blockIdx.y * BY + threadIdx.y;
     if (x0 >= d.nx || y >= d.ny) return;
-    for (int z = blockIdx.z; z < d.nz; z += gridDim.z) {
-        const size_t i0 = ((size_t)z * d.ny + y) * d.nx + x0;
+    for (int z = blockIdx.z * p.zper; z < min(d.nz, (int)(blockIdx.z + 1) * p.zper); ++z) {
+        const unsigned i0 = (unsigned)((z * d.ny + y) * d.nx + x0);
         float ux[VEC], uy[VEC], uz[VEC], o[VEC];
         load_vec<VEC>(p.u_in + i0, ux);
         load_vec<VEC>(p.u_in + N + i0, uy);
@@ -180,14 +181,14 @@ template <int VARIANT, int VEC>
 __global__ void __launch_bounds__(BX* BY) k_force_active(const KParams p) {
     if (skip_pass(p.sink)) return;
     const Dims d = p.d;
-    const size_t N = nvox(d);
+    const unsigned N = (unsigned)nvox(d);
     const int x0 = (blockIdx.x * BX + threadIdx.x) * VEC;
     const int y = blockIdx.y * BY + threadIdx.y;
     const bool active = x0 < d.nx && y < d.ny;
     double acc[3] = {0.0, 0.0, 0.0};
     if (active) {
-        for (int z = blockIdx.z; z < d.nz; z += gridDim.z) {
-            const size_t i0 = ((size_t)z * d.ny + y) * d.nx + x0;
+        for (int z = blockIdx.z * p.zper; z < min(d.nz, (int)(blockIdx.z + 1) * p.zper); ++z) {
+            const unsigned i0 = (unsigned)((z * d.ny + y) * d.nx + x0);
             float mw[VEC], ax[VEC], ay[VEC], az[VEC];  // warped moving image and its gradient
             centre_and_gradient<VEC>(p.Mw, d, x0, y, z, mw, ax, ay, az);
             float fx[VEC], fy[VEC], fz[VEC], dd[VEC];
@@ -236,8 +237,8 @@ __global__ void __launch_bounds__(BX* BY) k_force_active(const KParams p) {
 #pragma unroll
             for (int j = 0; j < VEC; ++j) {
                 ssd = fmaf(dd[j], dd[j], ssd);
-                sf += sqrtf(fmaf(fx[j], fx[j], fmaf(fy[j], fy[j], fz[j] * fz[j])));
-                su += sqrtf(fmaf(ux[j], ux[j], fmaf(uy[j], uy[j], uz[j] * uz[j])));
+                sf += fast_sqrt(fmaf(fx[j], fx[j], fmaf(fy[j], fy[j], fz[j] * fz[j])));
+                su += fast_sqrt(fmaf(ux[j], ux[j], fmaf(uy[j], uy[j], uz[j] * uz[j])));
                 ux[j] -= fx[j];
                 uy[j] -= fy[j];
                 uz[j] -= fz[j];
@@ -272,15 +273,12 @@ __global__ void __launch_bounds__(BX* BY) k_force_active(const KParams p) {
 
 bool aligned16(const void* p) { return p == nullptr || (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-constexpr int MAX_FORCE_BLOCKS = 65536;
+constexpr int ZPER = 4;  // planes per block: amortises the block reduction, keeps z neighbours in L1
 
 dim3 force_grid(const Dims& d, int vec) {
     const int gx = (d.nx + BX * vec - 1) / (BX * vec);
     const int gy = (d.ny + BY - 1) / BY;
-    int gz = d.nz;
-    const long long per_plane = (long long)gx * gy;
-    if (per_plane * gz > MAX_FORCE_BLOCKS) gz = (int)(MAX_FORCE_BLOCKS / per_plane);
-    if (gz < 1) gz = 1;
+    const int gz = (d.nz + ZPER - 1) / ZPER;
     return dim3(gx, gy, gz);
 }
 
@@ -337,6 +335,7 @@ int launch_warp_force(const ForceArgs& a, cudaStream_t st) {
     p.Sw = a.Sw;
     p.sink = a.sink;
     p.texM = a.texM;
+    p.zper = ZPER;
     const bool vec4 = (a.d.nx % 4 == 0) && aligned16(a.S) && aligned16(a.M) && aligned16(a.u_in) &&
                       aligned16(a.u_out) && aligned16(a.ub_in) && aligned16(a.ub_out) &&
                       aligned16(a.Mw) && aligned16(a.Sw);
