@@ -248,7 +248,7 @@ def main():
     smooth_launches = launches_per_iter - 1
     bytes_per_voxel = {"force": 32.0, "smooth": 24.0 if smooth_launches <= 1 else 72.0}
     kernel_names = {"force": "k_force_fixed<0> (fused warp+gradient+force+update+metrics)",
-                    "smooth": "k_smooth_fused (one pass, 3 components)" if smooth_launches <= 1
+                    "smooth": "k_smooth_tma (TMA-fed single pass, 3 components)" if smooth_launches <= 1
                     else "k_smooth_axis x3 (separable fallback, 3 components)"}
     peak, peak_src = measured_peak()
     per_kernel = {}

@@ -89,6 +89,7 @@ struct demons_ctx {
     int opt_profile = 0;
     int opt_smooth_zc = 0;
     int opt_no_tma = 0;
+    int opt_tune = 0;
     std::vector<cudaEvent_t> prof_all;                               // events of the profiled call
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_pairs[4];  // per kernel class: start/stop
     double prof_ms[4] = {0, 0, 0, 0};
@@ -322,6 +323,7 @@ int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb,
     sa.force_generic = c->opt_generic_smooth;
     sa.zc_override = c->opt_smooth_zc;
     sa.no_tma = c->opt_no_tma;
+    sa.tune = c->opt_tune;
     sa.in = fa.u_out;
     sa.out = lb.u;
     n = launch_smooth(sa, st);
@@ -560,6 +562,7 @@ int demons_set_option(demons_ctx* c, const char* name, int value) {
     else if (!strcmp(name, "profile")) c->opt_profile = value != 0;
     else if (!strcmp(name, "smooth_zc")) c->opt_smooth_zc = value;
     else if (!strcmp(name, "no_tma")) c->opt_no_tma = value != 0;
+    else if (!strcmp(name, "tune")) c->opt_tune = value;
     else return fail(DEMONS_E_ARG, "unknown option '%s'", name);
     for (auto& g : c->graphs) cudaGraphExecDestroy(g.exec);
     c->graphs.clear();
@@ -674,6 +677,7 @@ int demons_smooth(demons_ctx* c, const int dims[3], const float* d_in, float* d_
     sa.force_generic = c->opt_generic_smooth;
     sa.zc_override = c->opt_smooth_zc;
     sa.no_tma = c->opt_no_tma;
+    sa.tune = c->opt_tune;
     const int n = launch_smooth(sa, static_cast<cudaStream_t>(stream));
     if (n < 0) return fail(DEMONS_E_CUDA, "smooth launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     c->launches += n;

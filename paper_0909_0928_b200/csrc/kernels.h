@@ -40,6 +40,7 @@ struct SmoothArgs {
     int force_generic; // 1 = always use the three separable passes
     int zc_override;   // > 0: planes per CTA of the fused kernel (tuning)
     int no_tma;        // 1 = skip the TMA kernel (use the LDG-fed fused kernel)
+    int tune;          // kernel-configuration selector (tuning experiments; 0 = default)
 };
 int launch_smooth(const SmoothArgs& a, cudaStream_t stream);
 

@@ -18,6 +18,9 @@
 // kernel per axis through shared memory (L175), i.e. 24 B / element.
 #include <cuda.h>
 
+#include <cstdio>
+#include <cstdlib>
+
 #include "kernels.h"
 
 namespace demons {
@@ -85,8 +88,8 @@ struct Cfg {
     static_assert(TY >= R, "tile must be at least R rows high");
 };
 
-template <int R, int K, int RG, int STAGES>
-__global__ void __launch_bounds__(32 * (RG + 1))
+template <int R, int K, int RG, int STAGES, int MINB>
+__global__ void __launch_bounds__(32 * (RG + 1), MINB)
     k_smooth_tma(const __grid_constant__ CUtensorMap tmap, float* __restrict__ out, const Dims d, const int zc,
                  const int tiles_x, const Taps t, const int* __restrict__ skip) {
     using C = Cfg<R, K, RG, STAGES>;
@@ -270,7 +273,7 @@ EncodeTiledFn encode_fn() {
     return fn;
 }
 
-template <int R, int K, int RG, int STAGES>
+template <int R, int K, int RG, int STAGES, int MINB>
 int launch_cfg(const SmoothArgs& a, int zc, cudaStream_t st) {
     using C = Cfg<R, K, RG, STAGES>;
     EncodeTiledFn enc = encode_fn();
@@ -287,12 +290,21 @@ int launch_cfg(const SmoothArgs& a, int zc, cudaStream_t st) {
         return 0;
     static bool attr_set = false;
     if (!attr_set) {
-        if (cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM) !=
+        if (cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM) !=
             cudaSuccess) {
             cudaGetLastError();
             return 0;
         }
+        cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES, MINB>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
         attr_set = true;
+        if (getenv("DEMONS_DEBUG")) {
+            int nb = -1;
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_smooth_tma<R, K, RG, STAGES, MINB>, C::THREADS, C::SMEM);
+            cudaFuncAttributes fa;
+            cudaFuncGetAttributes(&fa, k_smooth_tma<R, K, RG, STAGES, MINB>);
+            fprintf(stderr, "[demons] k_smooth_tma<R=%d,K=%d,RG=%d>: %d regs, %d B dyn smem, %d threads -> %d CTAs/SM\n", R, K, RG,
+                    fa.numRegs, C::SMEM, C::THREADS, nb);
+        }
     }
     const int tiles_x = (d.nx + C::GX * 4 - 1) / (C::GX * 4);
     const int tiles_y = (d.ny + C::TY - 1) / C::TY;
@@ -301,7 +313,7 @@ int launch_cfg(const SmoothArgs& a, int zc, cudaStream_t st) {
     Taps t;
     for (int k = 0; k < 8; ++k) t.w[k] = k <= a.R ? a.w[k] : 0.f;
     const dim3 grid(tiles_x * tiles_y, chunks, a.ncomp);
-    k_smooth_tma<R, K, RG, STAGES><<<grid, C::THREADS, C::SMEM, st>>>(map, a.out, d, zc, tiles_x, t, a.skip);
+    k_smooth_tma<R, K, RG, STAGES, MINB><<<grid, C::THREADS, C::SMEM, st>>>(map, a.out, d, zc, tiles_x, t, a.skip);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
@@ -332,14 +344,22 @@ bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) ==
 int launch_smooth_tma(const SmoothArgs& a, cudaStream_t st) {
     if (a.d.nx % 4 != 0 || a.d.nx < 4 || !aligned16(a.in) || !aligned16(a.out)) return 0;
     if (a.R < 1 || a.R > 6) return 0;
-    const int zc = a.zc_override > 0 ? a.zc_override : pick_zc(a, 128, 16, 148 * 2);
+    // (tile height, CTAs per SM) of the configuration picked below
+    int tile_h = 8, per_sm = 3;
+    if (a.R == 4) per_sm = 2;
+    if (a.R > 4) tile_h = 16, per_sm = 1;
+    if (a.tune == 1) tile_h = 16, per_sm = 1;
+    const int zc = a.zc_override > 0 ? a.zc_override : pick_zc(a, 128, tile_h, 148 * per_sm);
+    if (a.tune == 1) {  // one large CTA per SM (tuning reference)
+        if (a.R == 3) return launch_cfg<3, 2, 8, 4, 1>(a, zc, st);
+    }
     switch (a.R) {
-    case 1: return launch_cfg<1, 2, 8, 4>(a, zc, st);
-    case 2: return launch_cfg<2, 2, 8, 4>(a, zc, st);
-    case 3: return launch_cfg<3, 2, 8, 4>(a, zc, st);
-    case 4: return launch_cfg<4, 2, 8, 4>(a, zc, st);
-    case 5: return launch_cfg<5, 2, 8, 3>(a, zc, st);
-    case 6: return launch_cfg<6, 2, 8, 3>(a, zc, st);
+    case 1: return launch_cfg<1, 2, 4, 4, 3>(a, zc, st);
+    case 2: return launch_cfg<2, 2, 4, 4, 3>(a, zc, st);
+    case 3: return launch_cfg<3, 2, 4, 4, 3>(a, zc, st);
+    case 4: return launch_cfg<4, 2, 4, 4, 2>(a, zc, st);
+    case 5: return launch_cfg<5, 2, 8, 3, 1>(a, zc, st);
+    case 6: return launch_cfg<6, 2, 8, 3, 1>(a, zc, st);
     default: return 0;
     }
 }
