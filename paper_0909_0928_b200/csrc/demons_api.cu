@@ -90,6 +90,8 @@ struct demons_ctx {
     int opt_smooth_zc = 0;
     int opt_no_tma = 0;
     int opt_tune = 0;
+    int opt_force_zper = 0;
+    int opt_force_scalar = 0;
     std::vector<cudaEvent_t> prof_all;                               // events of the profiled call
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_pairs[4];  // per kernel class: start/stop
     double prof_ms[4] = {0, 0, 0, 0};
@@ -302,6 +304,8 @@ int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb,
     fa.Sw = ic ? reinterpret_cast<float*>(c->ws + p.Sw) : nullptr;
     fa.sink = make_sink(c, p, reinterpret_cast<double*>(c->ws + p.stats), true, eps);
     fa.texM = c->opt_texture ? c->tex : 0;
+    fa.zper = c->opt_force_zper;
+    fa.force_scalar = c->opt_force_scalar;
     cudaEvent_t e0 = prof_event(c, st, true);
     fa.ev_mid = c->variant >= DEMONS_ACTIVE ? prof_event(c, st, false) : nullptr;
     int n = launch_warp_force(fa, st);
@@ -563,6 +567,8 @@ int demons_set_option(demons_ctx* c, const char* name, int value) {
     else if (!strcmp(name, "smooth_zc")) c->opt_smooth_zc = value;
     else if (!strcmp(name, "no_tma")) c->opt_no_tma = value != 0;
     else if (!strcmp(name, "tune")) c->opt_tune = value;
+    else if (!strcmp(name, "force_zper")) c->opt_force_zper = value;
+    else if (!strcmp(name, "force_scalar")) c->opt_force_scalar = value != 0;
     else return fail(DEMONS_E_ARG, "unknown option '%s'", name);
     for (auto& g : c->graphs) cudaGraphExecDestroy(g.exec);
     c->graphs.clear();
@@ -641,6 +647,8 @@ int demons_warp_force(demons_ctx* c, const int dims[3], const float* d_static, c
     fa.Mw = reinterpret_cast<float*>(c->ws + p.Mw);
     fa.Sw = ic ? reinterpret_cast<float*>(c->ws + p.Sw) : nullptr;
     fa.sink = make_sink(c, p, d_metrics, false, 0.0);
+    fa.zper = c->opt_force_zper;
+    fa.force_scalar = c->opt_force_scalar;
     if (c->opt_texture) {
         rc = bind_texture(c, d, d_moving, st);
         if (rc != DEMONS_OK) return rc;

@@ -20,6 +20,8 @@ struct ForceArgs {
     MetricSink sink;
     cudaTextureObject_t texM;  // 0 = software trilinear (default)
     cudaEvent_t ev_mid;        // nullable: recorded between the warp and the force kernel (profiling)
+    int zper;                  // > 0: planes per block (tuning); 0 = default
+    int force_scalar;          // 1 = take the one-voxel-per-thread kernels even when 128-bit access applies
 };
 
 // S1-S4 (+S6).  Returns the number of kernels launched, or -1 with cudaGetLastError() set.

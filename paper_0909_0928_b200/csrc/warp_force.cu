@@ -80,12 +80,27 @@ __global__ void __launch_bounds__(BX* BY) k_force_fixed(const KParams p) {
     const bool active = x0 < d.nx && y < d.ny;
     double acc[3] = {0.0, 0.0, 0.0};
     if (active) {
-        for (int z = blockIdx.z * p.zper; z < min(d.nz, (int)(blockIdx.z + 1) * p.zper); ++z) {
-            const unsigned i0 = (unsigned)((z * d.ny + y) * d.nx + x0);
+        // the field of the next plane is fetched while this plane's gathers and arithmetic run
+        const int zb = blockIdx.z * p.zper, ze = min(d.nz, zb + p.zper);
+        const unsigned plane = (unsigned)(d.nx * d.ny);
+        unsigned i0 = (unsigned)((zb * d.ny + y) * d.nx + x0);
+        float nux[VEC], nuy[VEC], nuz[VEC];
+        load_vec<VEC>(p.u_in + i0, nux);
+        load_vec<VEC>(p.u_in + N + i0, nuy);
+        load_vec<VEC>(p.u_in + 2 * N + i0, nuz);
+        for (int z = zb; z < ze; ++z, i0 += plane) {
             float ux[VEC], uy[VEC], uz[VEC];
-            load_vec<VEC>(p.u_in + i0, ux);
-            load_vec<VEC>(p.u_in + N + i0, uy);
-            load_vec<VEC>(p.u_in + 2 * N + i0, uz);
+#pragma unroll
+            for (int j = 0; j < VEC; ++j) {
+                ux[j] = nux[j];
+                uy[j] = nuy[j];
+                uz[j] = nuz[j];
+            }
+            if (z + 1 < ze) {
+                load_vec<VEC>(p.u_in + i0 + plane, nux);
+                load_vec<VEC>(p.u_in + N + i0 + plane, nuy);
+                load_vec<VEC>(p.u_in + 2 * N + i0 + plane, nuz);
+            }
             float mw[VEC];
 #pragma unroll
             for (int j = 0; j < VEC; ++j) {
@@ -275,17 +290,17 @@ bool aligned16(const void* p) { return p == nullptr || (reinterpret_cast<uintptr
 
 constexpr int ZPER = 4;  // planes per block: amortises the block reduction, keeps z neighbours in L1
 
-dim3 force_grid(const Dims& d, int vec) {
+dim3 force_grid(const Dims& d, int vec, int zper = ZPER) {
     const int gx = (d.nx + BX * vec - 1) / (BX * vec);
     const int gy = (d.ny + BY - 1) / BY;
-    const int gz = (d.nz + ZPER - 1) / ZPER;
+    const int gz = (d.nz + zper - 1) / zper;
     return dim3(gx, gy, gz);
 }
 
 template <int VEC, bool TEX>
 int launch_t(const ForceArgs& a, const KParams& p, cudaStream_t st) {
     const dim3 block(BX, BY);
-    const dim3 grid = force_grid(a.d, VEC);
+    const dim3 grid = force_grid(a.d, VEC, p.zper);
     switch (a.variant) {
     case 0: k_force_fixed<0, VEC, TEX><<<grid, block, 0, st>>>(p); return 1;
     case 1: k_force_fixed<1, VEC, TEX><<<grid, block, 0, st>>>(p); return 1;
@@ -335,8 +350,17 @@ int launch_warp_force(const ForceArgs& a, cudaStream_t st) {
     p.Sw = a.Sw;
     p.sink = a.sink;
     p.texM = a.texM;
-    p.zper = ZPER;
-    const bool vec4 = (a.d.nx % 4 == 0) && aligned16(a.S) && aligned16(a.M) && aligned16(a.u_in) &&
+    // planes per block: at least ZPER (never more blocks than force_partial_blocks() promised),
+    // more on large volumes so that ~1800 blocks remain (L1 reuse along z, fewer block reductions)
+    {
+        const dim3 g = force_grid(a.d, 1, 1);
+        const long long per_plane4 = (long long)((a.d.nx + BX * 4 - 1) / (BX * 4)) * g.y;
+        int zper = (int)((per_plane4 * a.d.nz + 1799) / 1800);
+        if (zper < ZPER) zper = ZPER;
+        if (zper > 32) zper = 32;
+        p.zper = a.zper >= ZPER ? a.zper : zper;
+    }
+    const bool vec4 = !a.force_scalar && (a.d.nx % 4 == 0) && aligned16(a.S) && aligned16(a.M) && aligned16(a.u_in) &&
                       aligned16(a.u_out) && aligned16(a.ub_in) && aligned16(a.ub_out) &&
                       aligned16(a.Mw) && aligned16(a.Sw);
     int n;
