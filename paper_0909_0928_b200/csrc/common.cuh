@@ -41,21 +41,20 @@ __device__ __forceinline__ float lerpf(float a, float b, float t) { return fmaf(
 // i1 = min(i0 + 1, n - 1).
 //  * The split is taken on u, not on x + u: floor(x + u) = x + floor(u) for integer x and
 //    u - floor(u) is exact in fp32, so no bits of the fraction are lost to the magnitude of x.
-//  * floor without the conversion unit: for |u| <= 2^21, t = u + 1.5*2^23 has ulp 1, so
-//    t - 1.5*2^23 = rint(u) exactly and the low mantissa bits of t are that integer.
-//  * The clamp is taken on the two indices: when p is outside [0, n-1] both become the same edge
-//    voxel and lerp(a, a, f) = a exactly, which is what clamping p does.
-__device__ __forceinline__ void split_axis(int x, float u, int n, int& i0, int& i1, float& f) {
+//  * floor without the conversion unit: for |u| <= 2^21, t = u + 1.5*2^23 ROUNDED DOWN (add.rm) has
+//    ulp 1, so t - 1.5*2^23 = floor(u) exactly and the low mantissa bits of t are that integer.
+// floor_split returns i = x + floor(u) (unclamped) and f = u - floor(u).
+__device__ __forceinline__ int floor_split(int x, float u, float& f) {
     u = fminf(fmaxf(u, -2097152.f), 2097152.f);
-    const float t = u + 12582912.f;
-    float r = t - 12582912.f;
-    int i = __float_as_int(t) - 0x4B400000;
-    if (r > u) {
-        r -= 1.f;
-        i -= 1;
-    }
-    f = u - r;
-    i += x;
+    const float t = __fadd_rd(u, 12582912.f);
+    f = u - (t - 12582912.f);
+    return __float_as_int(t) - 0x4B400000 + x;
+}
+
+// Generic form: the clamp is taken on the two indices.  When p is outside [0, n-1] both become the
+// same edge voxel and lerp(a, a, f) = a exactly, which is what clamping p does.
+__device__ __forceinline__ void split_axis(int x, float u, int n, int& i0, int& i1, float& f) {
+    const int i = floor_split(x, u, f);
     i0 = min(max(i, 0), n - 1);
     i1 = min(max(i + 1, 0), n - 1);
 }
@@ -81,6 +80,68 @@ __device__ __forceinline__ float trilinear(const float* __restrict__ I, const Di
     const float a01 = lerpf(c001, c101, fx), a11 = lerpf(c011, c111, fx);
     const float b0 = lerpf(a00, a10, fy), b1 = lerpf(a01, a11, fy);
     return lerpf(b0, b1, fz);
+}
+
+// ---- cell form of the same sample (the fast kernels) --------------------------------------------
+// The 2x2x2 cell is addressed by ONE offset o (its low corner); the other seven values sit at fixed
+// distances (+1, +nx, +nx*ny), so a lane issues its eight loads from one base with no per-load
+// index arithmetic and no branch.  The clamp of O2 is folded into (index, fraction):
+//     i < 0      ->  cell 0,     f = 0   (the sample is voxel 0)
+//     i > n - 2  ->  cell n - 2, f = 1   (the sample is voxel n - 1)
+// lerp1 is exact at both ends (t = 0 -> a, t = 1 -> b), so these reproduce the clamped sample
+// bit for bit.  Needs n >= 2 on every axis (the launchers send degenerate volumes elsewhere).
+__device__ __forceinline__ float lerp1(float a, float b, float t) { return fmaf(t, b, fmaf(-t, a, a)); }
+
+__device__ __forceinline__ void clamp_cell_axis(int& i, float& f, int n) {
+    f = i < 0 ? 0.f : f;
+    f = i > n - 2 ? 1.f : f;
+    i = min(max(i, 0), n - 2);
+}
+
+// Cells of NV voxels (xs[j], y, z) of one lane.  The clamp arithmetic is skipped when no lane of
+// the warp needs it (warp-uniform test; only pure ALU code sits under the branch).
+template <int NV>
+__device__ __forceinline__ void make_cells(const Dims& d, const int (&xs)[NV], int y, int z, const float (&ux)[NV],
+                                           const float (&uy)[NV], const float (&uz)[NV], unsigned (&o)[NV],
+                                           float (&fx)[NV], float (&fy)[NV], float (&fz)[NV]) {
+    int ix[NV], iy[NV], iz[NV];
+    bool inside = true;
+#pragma unroll
+    for (int j = 0; j < NV; ++j) {
+        ix[j] = floor_split(xs[j], ux[j], fx[j]);
+        iy[j] = floor_split(y, uy[j], fy[j]);
+        iz[j] = floor_split(z, uz[j], fz[j]);
+        inside = inside && (unsigned)ix[j] < (unsigned)(d.nx - 1) && (unsigned)iy[j] < (unsigned)(d.ny - 1) &&
+                 (unsigned)iz[j] < (unsigned)(d.nz - 1);
+    }
+    if (!__all_sync(__activemask(), inside)) {
+#pragma unroll
+        for (int j = 0; j < NV; ++j) {
+            clamp_cell_axis(ix[j], fx[j], d.nx);
+            clamp_cell_axis(iy[j], fy[j], d.ny);
+            clamp_cell_axis(iz[j], fz[j], d.nz);
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < NV; ++j) o[j] = (unsigned)((iz[j] * d.ny + iy[j]) * d.nx + ix[j]);
+}
+
+// The eight loads of a cell, issued back to back (x fastest).
+__device__ __forceinline__ void load_cell(const float* __restrict__ I, const Dims& d, unsigned o, float (&c)[8]) {
+    const unsigned o01 = o + (unsigned)(d.nx * d.ny);
+    const float* r00 = I + o;
+    const float* r10 = I + (o + (unsigned)d.nx);
+    const float* r01 = I + o01;
+    const float* r11 = I + (o01 + (unsigned)d.nx);
+    c[0] = __ldg(r00), c[1] = __ldg(r00 + 1), c[2] = __ldg(r10), c[3] = __ldg(r10 + 1);
+    c[4] = __ldg(r01), c[5] = __ldg(r01 + 1), c[6] = __ldg(r11), c[7] = __ldg(r11 + 1);
+}
+
+// Interpolation along x, then y, then z (O2).
+__device__ __forceinline__ float lerp_cell(const float (&c)[8], float fx, float fy, float fz) {
+    const float a00 = lerp1(c[0], c[1], fx), a10 = lerp1(c[2], c[3], fx);
+    const float a01 = lerp1(c[4], c[5], fx), a11 = lerp1(c[6], c[7], fx);
+    return lerp1(lerp1(a00, a10, fy), lerp1(a01, a11, fy), fz);
 }
 
 // VEC consecutive floats along x: one 128-bit access when VEC == 4.

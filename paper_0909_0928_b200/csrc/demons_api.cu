@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -305,6 +306,7 @@ int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb,
     fa.sink = make_sink(c, p, reinterpret_cast<double*>(c->ws + p.stats), true, eps);
     fa.texM = c->opt_texture ? c->tex : 0;
     fa.zper = c->opt_force_zper;
+    fa.tune = c->opt_tune;
     fa.force_scalar = c->opt_force_scalar;
     cudaEvent_t e0 = prof_event(c, st, true);
     fa.ev_mid = c->variant >= DEMONS_ACTIVE ? prof_event(c, st, false) : nullptr;
@@ -506,6 +508,7 @@ int demons_create(demons_ctx** out, const int dims[3], const float spacing[3], i
     c->variant = variant;
     c->alpha = alpha;
     c->sigma = sigma;
+    if (const char* t = getenv("DEMONS_TUNE")) c->opt_tune = (int)strtol(t, nullptr, 0);  // tuning experiments
     *out = c;
     return DEMONS_OK;
 }
@@ -648,6 +651,7 @@ int demons_warp_force(demons_ctx* c, const int dims[3], const float* d_static, c
     fa.Sw = ic ? reinterpret_cast<float*>(c->ws + p.Sw) : nullptr;
     fa.sink = make_sink(c, p, d_metrics, false, 0.0);
     fa.zper = c->opt_force_zper;
+    fa.tune = c->opt_tune;
     fa.force_scalar = c->opt_force_scalar;
     if (c->opt_texture) {
         rc = bind_texture(c, d, d_moving, st);

@@ -21,6 +21,7 @@ struct ForceArgs {
     cudaTextureObject_t texM;  // 0 = software trilinear (default)
     cudaEvent_t ev_mid;        // nullable: recorded between the warp and the force kernel (profiling)
     int zper;                  // > 0: planes per block (tuning); 0 = default
+    int tune;                  // kernel-layout selector (tuning experiments; 0 = default)
     int force_scalar;          // 1 = take the one-voxel-per-thread kernels even when 128-bit access applies
 };
 

@@ -157,6 +157,261 @@ __global__ void __launch_bounds__(BX* BY) k_force_fixed(const KParams p) {
     }
 }
 
+// ---- lane-consecutive kernels (the fast path) --------------------------------------------------
+// A warp owns a 32*XPT-wide stretch of one row; lane l owns the voxels x = xb + 32 j.  Every access
+// of a warp is then to 32 consecutive floats: the eight gathers of a voxel touch one or two
+// 128-byte lines per warp instead of the five that a float4-per-lane assignment touches (the L1
+// data pipe, not HBM, bounded that kernel).  All addresses of a row are (one 64-bit base) +
+// (128 j bytes), so the j loop costs no address arithmetic.  Per plane a lane issues, back to
+// back and with no branch in between, the field of the NEXT plane (register prefetch), the
+// stencil of S, and the 8 XPT gathers of M; it waits for memory once.  The centre value of S
+// rolls through registers along the z march.  FULL: nx is a multiple of 32*XPT (no ragged tail).
+template <int XPT, bool FULL>
+struct LcRow {
+    bool ok[XPT];  // voxel j exists
+    int dl0;       // 1 if voxel 0 has a left neighbour (x > 0); voxels j >= 1 always have one
+    int dr[XPT];   // 1 if voxel j has a right neighbour (x < nx - 1)
+    __device__ __forceinline__ LcRow(int xb, int nx) {
+        dl0 = xb > 0;
+#pragma unroll
+        for (int j = 0; j < XPT; ++j) {
+            ok[j] = FULL || xb + 32 * j < nx;
+            dr[j] = (FULL && j < XPT - 1) ? 1 : (xb + 32 * j < nx - 1);
+        }
+    }
+};
+
+// Raw stencil of I at the XPT voxels of a lane on plane z: x-1, x+1, y-1, y+1, z+1 (the values of
+// planes z-1 and z are already in registers).  Loads only; gradient_from_stencil does the math
+// after the gathers have been issued.
+template <int XPT>
+struct Stencil {
+    float xl[XPT], xr[XPT], ym[XPT], yp[XPT], zp[XPT];
+};
+
+template <int XPT, bool FULL>
+__device__ __forceinline__ void load_stencil(const float* __restrict__ I, const LcRow<XPT, FULL>& r, unsigned row,
+                                             unsigned dym, unsigned dyp, unsigned dzp, Stencil<XPT>& s) {
+    const float* pc = I + row;
+    const float* pl = I + (row - (unsigned)r.dl0);
+    const float* pym = I + (row - dym);
+    const float* pyp = I + (row + dyp);
+    const float* pzp = I + (row + dzp);
+#pragma unroll
+    for (int j = 0; j < XPT; ++j) {
+        if (FULL || r.ok[j]) {
+            s.xl[j] = j == 0 ? __ldg(pl) : __ldg(pc + 32 * j - 1);
+            s.xr[j] = (FULL && j < XPT - 1) ? __ldg(pc + 32 * j + 1) : __ldg(pc + 32 * j + r.dr[j]);
+            s.ym[j] = __ldg(pym + 32 * j);
+            s.yp[j] = __ldg(pyp + 32 * j);
+            s.zp[j] = __ldg(pzp + 32 * j);
+        } else {
+            s.xl[j] = s.xr[j] = s.ym[j] = s.yp[j] = s.zp[j] = 0.f;
+        }
+    }
+}
+
+// Everything a lane needs to finish one plane: the field, the raw stencil(s) and the gathered cells.
+template <int VARIANT, int XPT>
+struct PlaneRegs {
+    float ux[XPT], uy[XPT], uz[XPT];
+    Stencil<XPT> ss;
+    Stencil<VARIANT == 1 ? XPT : 1> ms;  // variant 1: stencil of the unwarped M (reading A4)
+    float c[XPT][8], fx[XPT], fy[XPT], fz[XPT];
+};
+
+// Software-pipelined along z: while plane z is computed, every load of plane z + 1 (stencil, the
+// 8 XPT gathers -- their addresses come from the field fetched one iteration earlier) and the field
+// of plane z + 2 are in flight, so a warp overlaps its own memory time with its own arithmetic and
+// the kernel does not depend on occupancy to hide HBM latency.  Two register sets (A/B) alternate.
+template <int VARIANT, int XPT, bool FULL, bool TEX, int MINB, bool PIPE>
+__global__ void __launch_bounds__(BX* BY, MINB) k_force_fixed_lc(const KParams p) {
+    if (skip_pass(p.sink)) return;
+    const Dims d = p.d;
+    const unsigned N = (unsigned)nvox(d);
+    const int xb = blockIdx.x * (32 * XPT) + threadIdx.x;
+    const int y = blockIdx.y * BY + threadIdx.y;
+    double acc[3] = {0.0, 0.0, 0.0};
+    if (xb < d.nx && y < d.ny) {
+        const LcRow<XPT, FULL> r(xb, d.nx);
+        int xs[XPT];  // a voxel past the ragged end samples the last voxel of the row (never stored)
+#pragma unroll
+        for (int j = 0; j < XPT; ++j) xs[j] = (FULL || r.ok[j]) ? xb + 32 * j : d.nx - 1;
+        const int zb = blockIdx.z * p.zper, ze = min(d.nz, zb + p.zper);
+        const unsigned plane = (unsigned)(d.nx * d.ny);
+        const unsigned row0 = (unsigned)((zb * d.ny + y) * d.nx + xb);
+        const unsigned dym = y > 0 ? (unsigned)d.nx : 0u, dyp = y < d.ny - 1 ? (unsigned)d.nx : 0u;
+        float nux[XPT], nuy[XPT], nuz[XPT];  // field of the plane after the one being issued
+        float sm[XPT], sc[XPT], mm[XPT], mc[XPT];  // centre values of planes z-1 and z (S; M for variant 1)
+
+        auto load_u = [&](unsigned row) {
+            const float *q0 = p.u_in + row, *q1 = p.u_in + (N + row), *q2 = p.u_in + (2 * N + row);
+#pragma unroll
+            for (int j = 0; j < XPT; ++j) {
+                const bool ok = FULL || r.ok[j];
+                nux[j] = ok ? __ldg(q0 + 32 * j) : 0.f;
+                nuy[j] = ok ? __ldg(q1 + 32 * j) : 0.f;
+                nuz[j] = ok ? __ldg(q2 + 32 * j) : 0.f;
+            }
+        };
+        // issue every load of plane z into q (its field is in nu*), then start fetching the field of z + 1
+        auto issue = [&](PlaneRegs<VARIANT, XPT>& q, int z) {
+            const unsigned row = row0 + (unsigned)(z - zb) * plane;
+#pragma unroll
+            for (int j = 0; j < XPT; ++j) {
+                q.ux[j] = nux[j];
+                q.uy[j] = nuy[j];
+                q.uz[j] = nuz[j];
+            }
+            if (z + 1 < ze) load_u(row + plane);
+            const unsigned dzp = z < d.nz - 1 ? plane : 0u;
+            load_stencil<XPT, FULL>(p.S, r, row, dym, dyp, dzp, q.ss);
+            if constexpr (VARIANT == 1) load_stencil<XPT, FULL>(p.M, r, row, dym, dyp, dzp, q.ms);
+            if constexpr (!TEX) {
+                unsigned o[XPT];
+                make_cells<XPT>(d, xs, y, z, q.ux, q.uy, q.uz, o, q.fx, q.fy, q.fz);
+#pragma unroll
+                for (int j = 0; j < XPT; ++j) load_cell(p.M, d, o[j], q.c[j]);
+            }
+        };
+        auto finish = [&](PlaneRegs<VARIANT, XPT>& q, int z) {
+            const unsigned row = row0 + (unsigned)(z - zb) * plane;
+            float* o0 = p.u_out + row;
+            float* o1 = p.u_out + (N + row);
+            float* o2 = p.u_out + (2 * N + row);
+            float ssd = 0.f, sf = 0.f, su = 0.f;
+#pragma unroll
+            for (int j = 0; j < XPT; ++j) {
+                float mw;
+                if constexpr (TEX)
+                    mw = tex3D<float>(p.texM, xs[j] + q.ux[j] + 0.5f, y + q.uy[j] + 0.5f, z + q.uz[j] + 0.5f);
+                else
+                    mw = lerp_cell(q.c[j], q.fx[j], q.fy[j], q.fz[j]);
+                const float gx = 0.5f * (q.ss.xr[j] - q.ss.xl[j]), gy = 0.5f * (q.ss.yp[j] - q.ss.ym[j]),
+                            gz = 0.5f * (q.ss.zp[j] - sm[j]);
+                const float dd = mw - sc[j];
+                const float g2 = fmaf(gx, gx, fmaf(gy, gy, gz * gz));
+                sm[j] = sc[j];
+                sc[j] = q.ss.zp[j];
+                float k;
+                if constexpr (VARIANT == 0) {
+                    k = guarded_div(dd, fmaf(dd, dd, g2));  // Eq.(1)
+                } else {
+                    // Eq.(2), gM0 = gradient of the UNWARPED level moving image (reading A4)
+                    const float hx = 0.5f * (q.ms.xr[j] - q.ms.xl[j]), hy = 0.5f * (q.ms.yp[j] - q.ms.ym[j]),
+                                hz = 0.5f * (q.ms.zp[j] - mm[j]);
+                    mm[j] = mc[j];
+                    mc[j] = q.ms.zp[j];
+                    const float m2 = fmaf(hx, hx, fmaf(hy, hy, hz * hz));
+                    const float num = 4.f * dd * fast_sqrt(g2) * fast_sqrt(m2);
+                    const float den = (fmaf(2.f * dd, dd, g2 + m2)) * (g2 + m2);
+                    k = guarded_div(num, den);
+                }
+                if (FULL || r.ok[j]) {
+                    o0[32 * j] = fmaf(-k, gx, q.ux[j]);
+                    o1[32 * j] = fmaf(-k, gy, q.uy[j]);
+                    o2[32 * j] = fmaf(-k, gz, q.uz[j]);
+                    ssd = fmaf(dd, dd, ssd);
+                    sf = fmaf(fabsf(k), fast_sqrt(g2), sf);  // |F| = |k| |gS|
+                    su += fast_sqrt(fmaf(q.ux[j], q.ux[j], fmaf(q.uy[j], q.uy[j], q.uz[j] * q.uz[j])));
+                }
+            }
+            acc[0] += (double)ssd;
+            acc[1] += (double)sf;
+            acc[2] += (double)su;
+        };
+
+        load_u(row0);
+        {
+            const float *qs = p.S + row0, *qsm = p.S + (row0 - (zb > 0 ? plane : 0u));
+            const float *qm = p.M + row0, *qmm = p.M + (row0 - (zb > 0 ? plane : 0u));
+#pragma unroll
+            for (int j = 0; j < XPT; ++j) {
+                const bool ok = FULL || r.ok[j];
+                sc[j] = ok ? __ldg(qs + 32 * j) : 0.f;
+                sm[j] = ok ? __ldg(qsm + 32 * j) : 0.f;
+                if constexpr (VARIANT == 1) {
+                    mc[j] = ok ? __ldg(qm + 32 * j) : 0.f;
+                    mm[j] = ok ? __ldg(qmm + 32 * j) : 0.f;
+                }
+            }
+        }
+        if constexpr (PIPE) {
+            PlaneRegs<VARIANT, XPT> A, B;
+            issue(A, zb);
+            for (int z = zb; z < ze; z += 2) {
+                if (z + 1 < ze) issue(B, z + 1);
+                finish(A, z);
+                if (z + 1 < ze) {
+                    if (z + 2 < ze) issue(A, z + 2);
+                    finish(B, z + 1);
+                }
+            }
+        } else {
+            PlaneRegs<VARIANT, XPT> A;
+            for (int z = zb; z < ze; ++z) {
+                issue(A, z);
+                finish(A, z);
+            }
+        }
+    }
+    if (p.sink.out != nullptr) {
+        if (block_reduce_publish<3>(acc, p.sink.partials, p.sink.stride, p.sink.ticket))
+            publish_metrics(acc, p.sink);
+    }
+}
+
+// Pass 1 of variants 2-5 in the same layout: Mw = warp(M, u)  (variant 5 also Sw = warp(S, ub)).
+template <int XPT, bool FULL, bool IC, bool TEX>
+__global__ void __launch_bounds__(BX* BY) k_warp_lc(const KParams p) {
+    if (skip_pass(p.sink)) return;
+    const Dims d = p.d;
+    const unsigned N = (unsigned)nvox(d);
+    const int xb = blockIdx.x * (32 * XPT) + threadIdx.x;
+    const int y = blockIdx.y * BY + threadIdx.y;
+    if (xb >= d.nx || y >= d.ny) return;
+    const LcRow<XPT, FULL> r(xb, d.nx);
+    int xs[XPT];
+#pragma unroll
+    for (int j = 0; j < XPT; ++j) xs[j] = (FULL || r.ok[j]) ? xb + 32 * j : d.nx - 1;
+    const int zb = blockIdx.z * p.zper, ze = min(d.nz, zb + p.zper);
+    const unsigned plane = (unsigned)(d.nx * d.ny);
+    unsigned row = (unsigned)((zb * d.ny + y) * d.nx + xb);
+    for (int z = zb; z < ze; ++z, row += plane) {
+#pragma unroll
+        for (int pass = 0; pass < (IC ? 2 : 1); ++pass) {
+            const float* u = pass == 0 ? p.u_in : p.ub_in;
+            const float* I = pass == 0 ? p.M : p.S;
+            float* out = (pass == 0 ? p.Mw : p.Sw) + row;
+            const float *q0 = u + row, *q1 = u + (N + row), *q2 = u + (2 * N + row);
+            float ux[XPT], uy[XPT], uz[XPT], v[XPT];
+#pragma unroll
+            for (int j = 0; j < XPT; ++j) {
+                const bool ok = FULL || r.ok[j];
+                ux[j] = ok ? __ldg(q0 + 32 * j) : 0.f;
+                uy[j] = ok ? __ldg(q1 + 32 * j) : 0.f;
+                uz[j] = ok ? __ldg(q2 + 32 * j) : 0.f;
+            }
+            if (TEX && pass == 0) {
+#pragma unroll
+                for (int j = 0; j < XPT; ++j)
+                    v[j] = tex3D<float>(p.texM, xs[j] + ux[j] + 0.5f, y + uy[j] + 0.5f, z + uz[j] + 0.5f);
+            } else {
+                unsigned o[XPT];
+                float fx[XPT], fy[XPT], fz[XPT], c[XPT][8];
+                make_cells<XPT>(d, xs, y, z, ux, uy, uz, o, fx, fy, fz);
+#pragma unroll
+                for (int j = 0; j < XPT; ++j) load_cell(I, d, o[j], c[j]);
+#pragma unroll
+                for (int j = 0; j < XPT; ++j) v[j] = lerp_cell(c[j], fx[j], fy[j], fz[j]);
+            }
+#pragma unroll
+            for (int j = 0; j < XPT; ++j)
+                if (FULL || r.ok[j]) out[32 * j] = v[j];
+        }
+    }
+}
+
 // ---- variants 2-5, pass 1: Mw = warp(M, u)  (variant 5 also Sw = warp(S, ub)) -----------------
 template <int VEC, bool IC, bool TEX>
 __global__ void __launch_bounds__(BX* BY) k_warp(const KParams p) {
@@ -328,6 +583,111 @@ int launch_t(const ForceArgs& a, const KParams& p, cudaStream_t st) {
     }
 }
 
+// Lane-consecutive kernels for the passes that gather; the stencil-only force pass of variants 2-5
+// keeps the float4 kernels when 128-bit access applies.
+// Planes per block of a marching kernel: the number of z chunks that minimises
+// (waves of blocks) x (planes per chunk + 2 planes of ring warm-up).  One wave of blocks that each
+// march a long chunk beats many short blocks: 59 us against 65 us at 256x256x100 (4 chunks of 25).
+int sm_count() {
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+    }
+    return n;
+}
+
+template <typename K>
+int pick_zper(K kernel, const dim3& tiles, int nz, int threads, int override_zper) {
+    if (override_zper >= ZPER) return override_zper;
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, 0) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError();
+        per_sm = 1;
+    }
+    const long long slots = (long long)sm_count() * per_sm, xy = (long long)tiles.x * tiles.y;
+    int best = nz < ZPER ? ZPER : nz;
+    long long best_cost = -1;
+    for (int chunks = 1; chunks <= nz; ++chunks) {
+        const int zper = (nz + chunks - 1) / chunks;
+        if (zper < ZPER) break;
+        const long long blocks = xy * ((nz + zper - 1) / zper);
+        const long long cost = ((blocks + slots - 1) / slots) * (zper + 2);
+        if (best_cost < 0 || cost < best_cost) {
+            best_cost = cost;
+            best = zper;
+        }
+    }
+    return best;
+}
+
+// Lane-consecutive kernels for the passes that gather; the stencil-only force pass of variants 2-5
+// keeps the float4 kernels when 128-bit access applies.
+template <int XPT, bool FULL, bool TEX, int MINB, bool PIPE = false>
+int launch_lc(const ForceArgs& a, const KParams& p0, bool vec4, cudaStream_t st) {
+    const dim3 block(BX, BY);
+    const dim3 tiles((a.d.nx + 32 * XPT - 1) / (32 * XPT), (a.d.ny + BY - 1) / BY, 1);
+    KParams p = p0;
+    auto grid_of = [&](int zper) { return dim3(tiles.x, tiles.y, (a.d.nz + zper - 1) / zper); };
+    if (a.variant == 0) {
+        p.zper = pick_zper(k_force_fixed_lc<0, XPT, FULL, TEX, MINB, PIPE>, tiles, a.d.nz, BX * BY, a.zper);
+        k_force_fixed_lc<0, XPT, FULL, TEX, MINB, PIPE><<<grid_of(p.zper), block, 0, st>>>(p);
+        return 1;
+    }
+    if (a.variant == 1) {
+        p.zper = pick_zper(k_force_fixed_lc<1, XPT, FULL, TEX, MINB, PIPE>, tiles, a.d.nz, BX * BY, a.zper);
+        k_force_fixed_lc<1, XPT, FULL, TEX, MINB, PIPE><<<grid_of(p.zper), block, 0, st>>>(p);
+        return 1;
+    }
+    if (a.variant == 5) {
+        p.zper = pick_zper(k_warp_lc<XPT, FULL, true, TEX>, tiles, a.d.nz, BX * BY, a.zper);
+        k_warp_lc<XPT, FULL, true, TEX><<<grid_of(p.zper), block, 0, st>>>(p);
+    } else {
+        p.zper = pick_zper(k_warp_lc<XPT, FULL, false, TEX>, tiles, a.d.nz, BX * BY, a.zper);
+        k_warp_lc<XPT, FULL, false, TEX><<<grid_of(p.zper), block, 0, st>>>(p);
+    }
+    if (a.ev_mid) cudaEventRecord(a.ev_mid, st);
+    p = p0;
+    const dim3 agrid = force_grid(a.d, vec4 ? 4 : 1, p.zper);
+    switch (a.variant) {
+    case 2: if (vec4) k_force_active<2, 4><<<agrid, block, 0, st>>>(p); else k_force_active<2, 1><<<agrid, block, 0, st>>>(p); break;
+    case 3: if (vec4) k_force_active<3, 4><<<agrid, block, 0, st>>>(p); else k_force_active<3, 1><<<agrid, block, 0, st>>>(p); break;
+    case 4: if (vec4) k_force_active<4, 4><<<agrid, block, 0, st>>>(p); else k_force_active<4, 1><<<agrid, block, 0, st>>>(p); break;
+    case 5: if (vec4) k_force_active<5, 4><<<agrid, block, 0, st>>>(p); else k_force_active<5, 1><<<agrid, block, 0, st>>>(p); break;
+    default: return -1;
+    }
+    return 2;
+}
+
+template <bool TEX>
+int launch_lc_x(const ForceArgs& a, const KParams& p, bool vec4, cudaStream_t st) {
+    int xpt = a.d.nx <= 32 ? 1 : a.d.nx <= 64 ? 2 : 4;
+    int minb = 2;
+    if constexpr (!TEX) {  // tuning experiments
+        if ((a.tune >> 4) & 0xF) xpt = (a.tune >> 4) & 0xF;
+        if ((a.tune >> 8) & 0xF) minb = (a.tune >> 8) & 0xF;
+        if (a.d.nx % (32 * xpt) == 0) {
+            if (xpt == 8 && minb == 1) return launch_lc<8, true, TEX, 1>(a, p, vec4, st);
+            if (xpt == 4 && minb == 1) return launch_lc<4, true, TEX, 1>(a, p, vec4, st);
+            if (xpt == 4 && minb == 3) return launch_lc<4, true, TEX, 3>(a, p, vec4, st);
+            if (xpt == 2 && minb == 3) return launch_lc<2, true, TEX, 3>(a, p, vec4, st);
+            if (xpt == 2 && minb == 4) return launch_lc<2, true, TEX, 4>(a, p, vec4, st);
+            if (xpt == 1 && minb == 4) return launch_lc<1, true, TEX, 4>(a, p, vec4, st);
+            if (xpt == 1 && minb == 6) return launch_lc<1, true, TEX, 6>(a, p, vec4, st);
+            if (xpt == 2 && minb == 9) return launch_lc<2, true, TEX, 2, true>(a, p, vec4, st);
+        }
+    }
+    if (a.d.nx % (32 * xpt) == 0) {
+        if (xpt == 1) return launch_lc<1, true, TEX, 2>(a, p, vec4, st);
+        if (xpt == 2) return launch_lc<2, true, TEX, 2>(a, p, vec4, st);
+        return launch_lc<4, true, TEX, 2>(a, p, vec4, st);
+    }
+    if (xpt == 1) return launch_lc<1, false, TEX, 2>(a, p, vec4, st);
+    if (xpt == 2) return launch_lc<2, false, TEX, 2>(a, p, vec4, st);
+    return launch_lc<4, false, TEX, 2>(a, p, vec4, st);
+}
+
 }  // namespace
 
 int force_partial_blocks(const Dims& d) {
@@ -364,7 +724,10 @@ int launch_warp_force(const ForceArgs& a, cudaStream_t st) {
                       aligned16(a.u_out) && aligned16(a.ub_in) && aligned16(a.ub_out) &&
                       aligned16(a.Mw) && aligned16(a.Sw);
     int n;
-    if (a.texM != 0)
+    const bool cells_ok = a.d.nx >= 2 && a.d.ny >= 2 && a.d.nz >= 2;  // make_cells needs a 2x2x2 cell
+    if ((a.tune & 0xF) != 2 && cells_ok)
+        n = a.texM != 0 ? launch_lc_x<true>(a, p, vec4, st) : launch_lc_x<false>(a, p, vec4, st);
+    else if (a.texM != 0)
         n = vec4 ? launch_t<4, true>(a, p, st) : launch_t<1, true>(a, p, st);
     else
         n = vec4 ? launch_t<4, false>(a, p, st) : launch_t<1, false>(a, p, st);
