@@ -88,8 +88,10 @@ __device__ __forceinline__ float trilinear(const float* __restrict__ I, const Di
 // index arithmetic and no branch.  The clamp of O2 is folded into (index, fraction):
 //     i < 0      ->  cell 0,     f = 0   (the sample is voxel 0)
 //     i > n - 2  ->  cell n - 2, f = 1   (the sample is voxel n - 1)
-// lerp1 is exact at both ends (t = 0 -> a, t = 1 -> b), so these reproduce the clamped sample
-// bit for bit.  Needs n >= 2 on every axis (the launchers send degenerate volumes elsewhere).
+// lerp1 is exact at both ends (t = 0 -> a, t = 1 -> b), so these reproduce the clamped sample bit for
+// bit -- with fma(t, b - a, a) the t = 1 case returns a + (b - a) != b and identical volumes would no
+// longer give exactly zero force at the high faces (pin P1).  lerp1 costs one more rounding per level.
+// Needs n >= 2 on every axis (the launchers send degenerate volumes elsewhere).
 __device__ __forceinline__ float lerp1(float a, float b, float t) { return fmaf(t, b, fmaf(-t, a, a)); }
 
 __device__ __forceinline__ void clamp_cell_axis(int& i, float& f, int n) {

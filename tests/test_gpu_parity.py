@@ -348,3 +348,92 @@ def test_api_rejects_bad_calls(torch_cuda, B):
         B.demons_smooth(eng.ctx, dims, f, f.clone(), 3, 20.0)
     assert e.value.code == B.E_UNSUPPORTED
     eng.close()
+
+
+# ---- full size: BASELINE.json config 2 shapes, the launch configuration bench.py times ----------
+FULL_DIMS = (256, 256, 100)
+
+
+@pytest.fixture(scope="module")
+def lung_case(P):
+    """The bench pair plus a live field: the analytic breathing field scaled down (a field a few
+    voxels large, smooth, non-zero at every border)."""
+    S, M, truth = P.lung_pair(FULL_DIMS, 202)
+    u = (0.35 * truth).astype(np.float32)
+    return S, M, u
+
+
+def force_atol(oracle, variant, S, M, u, ub):
+    """Per-voxel absolute tolerance of u_out at HU-scale intensities (tolerance derivation).
+    Eq.(1)-(6) are d g / (d^2 + |g|^2) terms: |dF/dd| reaches 1/|g| at d = 0, and d = Mw - S carries
+    the fp32 rounding of the trilinear sample, up to 2 ulp(|I|max) against the oracle's fp64 lerp.
+    Where the gradient is below ~1 HU/voxel that alone exceeds 1e-4, so the bound is
+    1e-4 + 4 ulp * (sum over the force terms of 1/|g|), capped at 1 (|F| <= 1)."""
+    def norm(g):
+        return np.sqrt((g.astype(np.float64) ** 2).sum(axis=0))
+    ulp = float(np.spacing(np.float32(max(np.abs(S).max(), np.abs(M).max()))))
+    tiny = 1e-12
+    gS = norm(oracle.gradient(S))
+    if variant == 0:
+        sens = 1.0 / np.maximum(gS, tiny)
+    elif variant == 1:
+        sens = 4.0 / np.maximum(np.sqrt(gS ** 2 + norm(oracle.gradient(M)) ** 2), tiny)
+    else:
+        Mw = oracle.warp(M, u)
+        if variant == 5:
+            G = oracle.gradient(Mw).astype(np.float64) + oracle.gradient(oracle.warp(S, ub)).astype(np.float64)
+            sens = 2.0 / np.maximum(np.sqrt((G ** 2).sum(axis=0)), tiny)
+        else:
+            sens = 2.0 / np.maximum(norm(oracle.gradient(Mw)), tiny)
+            if variant in (3, 4):
+                sens = sens + 1.0 / np.maximum(gS, tiny)
+    return np.minimum(1e-4 + 4.0 * ulp * sens, 1.0)[None]
+
+
+@pytest.mark.parametrize("variant", [0, 1, 3, 5])
+def test_full_size_warp_force_matches_oracle(torch_cuda, B, oracle, lung_case, variant):
+    """Every voxel of the 256x256x100 pass (the oracle takes about a second per call)."""
+    torch = torch_cuda
+    S, M, u = lung_case
+    ic = variant == 5
+    ub = (-u).copy()
+    ref_u, ref_ub, ref_m = oracle.warp_force(variant, 1.0, S, M, u, ub if ic else None)
+    eng = B.Demons(FULL_DIMS, variant=variant)
+    du = dev(torch, u)
+    out = torch.full_like(du, float("nan"))
+    outb = torch.full_like(du, float("nan")) if ic else None
+    met = torch.zeros(3, dtype=torch.float64, device="cuda:0")
+    B.demons_warp_force(eng.ctx, FULL_DIMS, dev(torch, S), dev(torch, M), du, out, dev(torch, ub) if ic else None,
+                        outb, met)
+    torch.cuda.synchronize()
+    atol = force_atol(oracle, variant, S, M, u, ub)
+    assert float((atol > 1e-3).mean()) < 1e-3  # the conditioning term matters for a handful of voxels only
+    assert_close(out.cpu().numpy(), ref_u, f"full-size u_out variant {variant}", atol=atol)
+    if ic:
+        assert_close(outb.cpu().numpy(), ref_ub, "full-size ub_out", atol=atol)
+    np.testing.assert_allclose(met.cpu().numpy(), ref_m, rtol=1e-5)
+    eng.close()
+
+
+@pytest.mark.parametrize("sigma", [1.0, 2.0])
+def test_full_size_smooth_matches_oracle(torch_cuda, B, oracle, sigma):
+    torch = torch_cuda
+    rng = np.random.default_rng(23)
+    f = (rng.standard_normal((3, FULL_DIMS[2], FULL_DIMS[1], FULL_DIMS[0])) * 4.0).astype(np.float32)
+    ref = oracle.smooth(f, sigma)
+    eng = B.Demons(FULL_DIMS)
+    out = torch.full((3, FULL_DIMS[2], FULL_DIMS[1], FULL_DIMS[0]), float("nan"), dtype=torch.float32, device="cuda:0")
+    B.demons_smooth(eng.ctx, FULL_DIMS, dev(torch, f), out, 3, sigma)
+    torch.cuda.synchronize()
+    assert_close(out.cpu().numpy(), ref, f"full-size smooth sigma {sigma}")
+    eng.close()
+
+
+def test_full_size_registration_prefix_matches_oracle(torch_cuda, B, oracle, lung_case):
+    """The first iterations of the bench registration (graph replay, same launch configuration):
+    field within 1e-2 voxel, per-iteration metrics within 2e-4 relative."""
+    S, M, _ = lung_case
+    iters = [4]
+    ref = oracle.register(0, 1.0, 1.0, S, M, iters)
+    res = run_register(torch_cuda, B, 0, S, M, iters)
+    check_registration(res, ref, "config 2 prefix")
