@@ -16,12 +16,11 @@
 // clamped when the shared-memory addresses are formed.
 // HBM sees every element once in and once out (8 B / element); the paper's design was one
 // kernel per axis through shared memory (L175), i.e. 24 B / element.
-#include <cuda.h>
-
 #include <cstdio>
 #include <cstdlib>
 
 #include "kernels.h"
+#include "tma.cuh"
 
 namespace demons {
 
@@ -31,34 +30,9 @@ struct Taps {
     float w[8];
 };
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)),
-        "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2,
-                                            int c3) {
-    asm volatile(
-        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
-        ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
-        : "memory");
-}
+using tma::mbar_expect_tx;
+using tma::mbar_init;
+using tma::mbar_wait;
 
 struct F4 {  // a float4 as two packed pairs
     float2 a, b;
@@ -144,13 +118,12 @@ __global__ void __launch_bounds__(32 * (RG + 1), MINB)
         const int s = p % STAGES;
         const int z = min(max(z_start - R + p, 0), d.nz - 1);
         mbar_expect_tx(&full[s], (uint32_t)(C::ROWS * BOXW * 4));
-        tma_load_4d(smem + s * C::STAGE_BYTES, &tmap, &full[s], x0 - 4 * NH, y0 - R, z, comp);
+        tma::load_4d(smem + s * C::STAGE_BYTES, &tmap, &full[s], x0 - 4 * NH, y0 - R, z, comp);
     };
     if (issuer) {
 #pragma unroll
         for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        tma::mbar_fence_init();
     }
     __syncthreads();
     if (issuer) {
@@ -253,41 +226,15 @@ __global__ void __launch_bounds__(32 * (RG + 1), MINB)
     }
 }
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-EncodeTiledFn encode_fn() {
-    static EncodeTiledFn fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-            q == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<EncodeTiledFn>(p);
-        else
-            cudaGetLastError();
-    }
-    return fn;
-}
-
 template <int R, int K, int RG, int STAGES, int MINB>
 int launch_cfg(const SmoothArgs& a, int zc, cudaStream_t st) {
     using C = Cfg<R, K, RG, STAGES>;
-    EncodeTiledFn enc = encode_fn();
-    if (!enc) return 0;
     const Dims d = a.d;
     alignas(64) CUtensorMap map;
-    const cuuint64_t gdim[4] = {(cuuint64_t)d.nx, (cuuint64_t)d.ny, (cuuint64_t)d.nz, (cuuint64_t)a.ncomp};
-    const cuuint64_t gstr[3] = {(cuuint64_t)d.nx * 4, (cuuint64_t)d.nx * d.ny * 4, (cuuint64_t)d.nx * d.ny * d.nz * 4};
-    const cuuint32_t box[4] = {(cuuint32_t)C::BOXW, (cuuint32_t)C::ROWS, 1, 1};
-    const cuuint32_t estr[4] = {1, 1, 1, 1};
-    if (enc(&map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, const_cast<float*>(a.in), gdim, gstr, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-        return 0;
+    const unsigned long long gdim[4] = {(unsigned long long)d.nx, (unsigned long long)d.ny, (unsigned long long)d.nz,
+                                        (unsigned long long)a.ncomp};
+    const unsigned box[4] = {(unsigned)C::BOXW, (unsigned)C::ROWS, 1u, 1u};
+    if (!tma::encode_f32(&map, a.in, 4, gdim, box)) return 0;
     static bool attr_set = false;
     if (!attr_set) {
         if (cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM) !=

@@ -232,7 +232,7 @@ __global__ void __launch_bounds__(BX* BY, MINB) k_force_fixed_lc(const KParams p
     const Dims d = p.d;
     const unsigned N = (unsigned)nvox(d);
     const int xb = blockIdx.x * (32 * XPT) + threadIdx.x;
-    const int y = blockIdx.y * BY + threadIdx.y;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
     double acc[3] = {0.0, 0.0, 0.0};
     if (xb < d.nx && y < d.ny) {
         const LcRow<XPT, FULL> r(xb, d.nx);
@@ -360,7 +360,7 @@ __global__ void __launch_bounds__(BX* BY) k_warp_lc(const KParams p) {
     const Dims d = p.d;
     const unsigned N = (unsigned)nvox(d);
     const int xb = blockIdx.x * (32 * XPT) + threadIdx.x;
-    const int y = blockIdx.y * BY + threadIdx.y;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
     if (xb >= d.nx || y >= d.ny) return;
     const LcRow<XPT, FULL> r(xb, d.nx);
     int xs[XPT];
@@ -575,11 +575,6 @@ int launch_t(const ForceArgs& a, const KParams& p, cudaStream_t st) {
     }
 }
 
-// Lane-consecutive kernels for the passes that gather; the stencil-only force pass of variants 2-5
-// keeps the float4 kernels when 128-bit access applies.
-// Planes per block of a marching kernel: the number of z chunks that minimises
-// (waves of blocks) x (planes per chunk + 2 planes of ring warm-up).  One wave of blocks that each
-// march a long chunk beats many short blocks: 59 us against 65 us at 256x256x100 (4 chunks of 25).
 int sm_count() {
     static int n = 0;
     if (n == 0) {
@@ -590,25 +585,37 @@ int sm_count() {
     return n;
 }
 
+// Block shape of a marching kernel: rows per block (4..8 warps) and planes per block, chosen to
+// minimise  (waves of blocks) x (rows per block) x (planes per chunk + 2 planes of ring warm-up),
+// i.e. the work of the busiest SM.  One wave of long marches beats many short blocks (59 against 65 us
+// at 256x256x100), and a wave that fills every slot beats one that leaves SMs half empty: 8-row blocks
+// give 256 blocks for 296 slots there, 7-row blocks give exactly 296.
+struct Shape {
+    int by, zper;
+};
+
 template <typename K>
-int pick_zper(K kernel, const dim3& tiles, int nz, int threads, int override_zper) {
-    if (override_zper >= ZPER) return override_zper;
-    int per_sm = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, 0) != cudaSuccess || per_sm < 1) {
-        cudaGetLastError();
-        per_sm = 1;
-    }
-    const long long slots = (long long)sm_count() * per_sm, xy = (long long)tiles.x * tiles.y;
-    int best = nz < ZPER ? ZPER : nz;
+Shape pick_shape(K kernel, int tiles_x, int ny, int nz, int override_zper) {
+    Shape best{BY, nz < ZPER ? ZPER : nz};
     long long best_cost = -1;
-    for (int chunks = 1; chunks <= nz; ++chunks) {
-        const int zper = (nz + chunks - 1) / chunks;
-        if (zper < ZPER) break;
-        const long long blocks = xy * ((nz + zper - 1) / zper);
-        const long long cost = ((blocks + slots - 1) / slots) * (zper + 2);
-        if (best_cost < 0 || cost < best_cost) {
-            best_cost = cost;
-            best = zper;
+    for (int by = BY; by >= 4; --by) {
+        int per_sm = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, BX * by, 0) != cudaSuccess || per_sm < 1) {
+            cudaGetLastError();
+            per_sm = 1;
+        }
+        const long long slots = (long long)sm_count() * per_sm, xy = (long long)tiles_x * ((ny + by - 1) / by);
+        for (int chunks = 1; chunks <= nz; ++chunks) {
+            int zper = (nz + chunks - 1) / chunks;
+            if (override_zper >= ZPER) zper = override_zper;
+            if (zper < ZPER) break;
+            const long long blocks = xy * ((nz + zper - 1) / zper);
+            const long long cost = ((blocks + slots - 1) / slots) * by * per_sm * (zper + 2);
+            if (best_cost < 0 || cost < best_cost) {
+                best_cost = cost;
+                best = Shape{by, zper};
+            }
+            if (override_zper >= ZPER) break;
         }
     }
     return best;
@@ -618,29 +625,27 @@ int pick_zper(K kernel, const dim3& tiles, int nz, int threads, int override_zpe
 // keeps the float4 kernels when 128-bit access applies.
 template <int XPT, bool FULL, bool TEX, int MINB>
 int launch_lc(const ForceArgs& a, const KParams& p0, bool vec4, cudaStream_t st) {
-    const dim3 block(BX, BY);
-    const dim3 tiles((a.d.nx + 32 * XPT - 1) / (32 * XPT), (a.d.ny + BY - 1) / BY, 1);
+    const int tiles_x = (a.d.nx + 32 * XPT - 1) / (32 * XPT);
     KParams p = p0;
-    auto grid_of = [&](int zper) { return dim3(tiles.x, tiles.y, (a.d.nz + zper - 1) / zper); };
+    auto run = [&](auto kernel) {
+        const Shape sh = pick_shape(kernel, tiles_x, a.d.ny, a.d.nz, a.zper);
+        p.zper = sh.zper;
+        const dim3 grid(tiles_x, (a.d.ny + sh.by - 1) / sh.by, (a.d.nz + sh.zper - 1) / sh.zper);
+        kernel<<<grid, dim3(BX, sh.by), 0, st>>>(p);
+    };
     if (a.variant == 0) {
-        p.zper = pick_zper(k_force_fixed_lc<0, XPT, FULL, TEX, MINB>, tiles, a.d.nz, BX * BY, a.zper);
-        k_force_fixed_lc<0, XPT, FULL, TEX, MINB><<<grid_of(p.zper), block, 0, st>>>(p);
+        run(k_force_fixed_lc<0, XPT, FULL, TEX, MINB>);
         return 1;
     }
     if (a.variant == 1) {
-        p.zper = pick_zper(k_force_fixed_lc<1, XPT, FULL, TEX, MINB>, tiles, a.d.nz, BX * BY, a.zper);
-        k_force_fixed_lc<1, XPT, FULL, TEX, MINB><<<grid_of(p.zper), block, 0, st>>>(p);
+        run(k_force_fixed_lc<1, XPT, FULL, TEX, MINB>);
         return 1;
     }
-    if (a.variant == 5) {
-        p.zper = pick_zper(k_warp_lc<XPT, FULL, true, TEX>, tiles, a.d.nz, BX * BY, a.zper);
-        k_warp_lc<XPT, FULL, true, TEX><<<grid_of(p.zper), block, 0, st>>>(p);
-    } else {
-        p.zper = pick_zper(k_warp_lc<XPT, FULL, false, TEX>, tiles, a.d.nz, BX * BY, a.zper);
-        k_warp_lc<XPT, FULL, false, TEX><<<grid_of(p.zper), block, 0, st>>>(p);
-    }
+    if (a.variant == 5) run(k_warp_lc<XPT, FULL, true, TEX>);
+    else run(k_warp_lc<XPT, FULL, false, TEX>);
     if (a.ev_mid) cudaEventRecord(a.ev_mid, st);
     p = p0;
+    const dim3 block(BX, BY);
     const dim3 agrid = force_grid(a.d, vec4 ? 4 : 1, p.zper);
     switch (a.variant) {
     case 2: if (vec4) k_force_active<2, 4><<<agrid, block, 0, st>>>(p); else k_force_active<2, 1><<<agrid, block, 0, st>>>(p); break;
@@ -672,9 +677,9 @@ int launch_lc_x(const ForceArgs& a, const KParams& p, bool vec4, cudaStream_t st
 }  // namespace
 
 int force_partial_blocks(const Dims& d) {
-    // the scalar grid is the larger of the two
-    const dim3 g = force_grid(d, 1);
-    return (int)(g.x * g.y * g.z);
+    // the largest grid any force kernel uses: 32-voxel tiles, 4-row blocks (pick_shape), ZPER planes
+    const long long gx = (d.nx + BX - 1) / BX, gy = (d.ny + 3) / 4, gz = (d.nz + ZPER - 1) / ZPER;
+    return (int)(gx * gy * gz);
 }
 
 int launch_warp_force(const ForceArgs& a, cudaStream_t st) {

@@ -1,7 +1,7 @@
 """BASELINE.json config 5: bandwidth sweep of the per-iteration kernels through the C ABI.
 
     python -m paper_0909_0928_b200.sweep [--sizes 128x128x64,256x256x100,...] [--reps 20]
-                                         [--kernels force,smooth,pyramid] [--json out.json]
+                                         [--kernels force,smooth,pyramid,texture] [--json out.json]
 
 For every size: the fused warp+force+update entry point for all six variants, the Gaussian
 smoothing at sigma 1.0 and 2.0 (3 components), restrict and prolong.  Inputs are the seeded blob
@@ -79,6 +79,22 @@ def run(sizes, kernels, reps, device="cuda:0"):
                     eng.ctx, dims, dS, dM, du, out, dub if ic else None, outb if ic else None, met, stream), reps)
                 add(f"warp_force[{VARIANT_NAMES[variant]}]", ms, FORCE_BYTES[variant] * N)
                 eng.close()
+        if "texture" in kernels:
+            # S9: hardware linear filtering (9-bit weights) against the software trilinear of the same pass
+            eng = B.Demons(dims, variant=0, device=device)
+            B.demons_warp_force(eng.ctx, dims, dS, dM, du, out, None, None, met, stream)
+            torch.cuda.synchronize()
+            soft = out.clone()
+            B.demons_set_option(eng.ctx, "texture", 1)
+            ms = median_ms(torch, stream, lambda: B.demons_warp_force(
+                eng.ctx, dims, dS, dM, du, out, None, None, met, stream), reps)
+            torch.cuda.synchronize()
+            err = (out - soft).abs()
+            add("warp_force[passive, texture unit]", ms, FORCE_BYTES[0] * N)
+            rows[-1]["max_abs_err_vs_software_voxel"] = float(err.max())
+            rows[-1]["mean_abs_err_vs_software_voxel"] = float(err.mean())
+            rows[-1]["frac_outside_1e-4"] = float((err > 1e-4).float().mean())
+            eng.close()
         eng = B.Demons(dims, variant=0, device=device)
         if "smooth" in kernels:
             for sigma in (1.0, 2.0):
@@ -99,7 +115,7 @@ def run(sizes, kernels, reps, device="cuda:0"):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--sizes", default="128x128x64,256x256x100,512x512x160,512x512x256")
-    ap.add_argument("--kernels", default="force,smooth,pyramid")
+    ap.add_argument("--kernels", default="force,smooth,pyramid,texture")
     ap.add_argument("--reps", type=int, default=20)
     ap.add_argument("--json", default=None)
     args = ap.parse_args()
@@ -108,7 +124,11 @@ def main():
     print(f"# HBM peak {peak:.1f} GB/s ({kind}); effective GB/s = algorithmic bytes / median time")
     print(f"{'dims':>12} {'kernel':<34} {'ms':>9} {'GB/s':>9} {'% peak':>7}")
     for r in rows:
-        print(f"{r['dims']:>12} {r['kernel']:<34} {r['ms']:9.4f} {r['gbs']:9.1f} {r['pct_of_peak']:7.1f}")
+        extra = ""
+        if "max_abs_err_vs_software_voxel" in r:
+            extra = (f"  |u'(tex) - u'(software)|: max {r['max_abs_err_vs_software_voxel']:.3e} mean "
+                     f"{r['mean_abs_err_vs_software_voxel']:.3e} voxel, {100 * r['frac_outside_1e-4']:.1f}% outside 1e-4")
+        print(f"{r['dims']:>12} {r['kernel']:<34} {r['ms']:9.4f} {r['gbs']:9.1f} {r['pct_of_peak']:7.1f}{extra}")
     if args.json:
         with open(args.json, "w") as fh:
             json.dump({"peak_gbs": peak, "peak_kind": kind, "rows": rows}, fh, indent=1)
