@@ -30,39 +30,51 @@ __global__ void __launch_bounds__(256) k_restrict(const float* __restrict__ fine
 
 // O7: fine voxel x sits at coarse coordinate (x - 0.5)/2, clamped to [0, n_c - 1];
 // u_f = 2 * trilinear(u_c) per component (factor 2: PAPER.md L123-125; alignment: reading A12).
-__device__ __forceinline__ void coarse_axis(int x, int nc, int& i0, int& i1, float& f) {
-    float p = 0.5f * ((float)x - 0.5f);
-    p = fminf(fmaxf(p, 0.f), (float)(nc - 1));
-    const float fl = floorf(p);
-    i0 = (int)fl;
-    f = p - fl;
-    i1 = min(i0 + 1, nc - 1);
-}
-
+// One thread per coarse CELL (i..i+1, j..j+1, k..k+1), i in [-1, n_c - 1]: the up to 2x2x2 fine voxels
+// x in {2i+1, 2i+2} x ... interpolate inside that one cell with the weights 1/4 (x = 2i+1) and 3/4
+// (x = 2i+2), so the 8 coarse values of a component are loaded once for 8 outputs.  At the faces the
+// clamp makes both cell corners the same voxel (i = -1 -> voxel 0, i = n_c - 1 -> voxel n_c - 1), which is
+// exactly what clamping the coarse coordinate does.  Interpolation order x, y, z as in O2.
 __global__ void __launch_bounds__(256) k_prolong(const float* __restrict__ uc, float* __restrict__ uf,
                                                  const Dims cd, const Dims fd) {
-    const int x = blockIdx.x * blockDim.x + threadIdx.x;
-    const int y = blockIdx.y * blockDim.y + threadIdx.y;
-    const int z = blockIdx.z;
-    if (x >= fd.nx || y >= fd.ny) return;
-    int x0, x1, y0, y1, z0, z1;
-    float fx, fy, fz;
-    coarse_axis(x, cd.nx, x0, x1, fx);
-    coarse_axis(y, cd.ny, y0, y1, fy);
-    coarse_axis(z, cd.nz, z0, z1, fz);
-    const size_t Nc = nvox(cd), Nf = nvox(fd);
-    const size_t o00 = ((size_t)z0 * cd.ny + y0) * cd.nx, o10 = ((size_t)z0 * cd.ny + y1) * cd.nx;
-    const size_t o01 = ((size_t)z1 * cd.ny + y0) * cd.nx, o11 = ((size_t)z1 * cd.ny + y1) * cd.nx;
-    const size_t of = ((size_t)z * fd.ny + y) * fd.nx + x;
+    const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x) - 1;
+    const int j = (int)(blockIdx.y * blockDim.y + threadIdx.y) - 1;
+    const int k = (int)blockIdx.z - 1;
+    if (i >= cd.nx || j >= cd.ny) return;
+    const int x0 = max(i, 0), x1 = min(i + 1, cd.nx - 1);
+    const int y0 = max(j, 0), y1 = min(j + 1, cd.ny - 1);
+    const int z0 = max(k, 0), z1 = min(k + 1, cd.nz - 1);
+    const unsigned Nc = (unsigned)nvox(cd), Nf = (unsigned)nvox(fd);
+    const unsigned o00 = (unsigned)((z0 * cd.ny + y0) * cd.nx), o10 = (unsigned)((z0 * cd.ny + y1) * cd.nx);
+    const unsigned o01 = (unsigned)((z1 * cd.ny + y0) * cd.nx), o11 = (unsigned)((z1 * cd.ny + y1) * cd.nx);
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         const float* I = uc + c * Nc;
-        const float a00 = lerpf(__ldg(I + o00 + x0), __ldg(I + o00 + x1), fx);
-        const float a10 = lerpf(__ldg(I + o10 + x0), __ldg(I + o10 + x1), fx);
-        const float a01 = lerpf(__ldg(I + o01 + x0), __ldg(I + o01 + x1), fx);
-        const float a11 = lerpf(__ldg(I + o11 + x0), __ldg(I + o11 + x1), fx);
-        const float b0 = lerpf(a00, a10, fy), b1 = lerpf(a01, a11, fy);
-        uf[c * Nf + of] = 2.f * lerpf(b0, b1, fz);
+        const float c000 = __ldg(I + o00 + x0), c100 = __ldg(I + o00 + x1), c010 = __ldg(I + o10 + x0),
+                    c110 = __ldg(I + o10 + x1), c001 = __ldg(I + o01 + x0), c101 = __ldg(I + o01 + x1),
+                    c011 = __ldg(I + o11 + x0), c111 = __ldg(I + o11 + x1);
+#pragma unroll
+        for (int dz = 1; dz <= 2; ++dz) {
+            const int z = 2 * k + dz;
+            if (z < 0 || z >= fd.nz) continue;
+            const float fz = dz == 1 ? 0.25f : 0.75f;
+#pragma unroll
+            for (int dy = 1; dy <= 2; ++dy) {
+                const int y = 2 * j + dy;
+                if (y < 0 || y >= fd.ny) continue;
+                const float fy = dy == 1 ? 0.25f : 0.75f;
+#pragma unroll
+                for (int dx = 1; dx <= 2; ++dx) {
+                    const int x = 2 * i + dx;
+                    if (x < 0 || x >= fd.nx) continue;
+                    const float fx = dx == 1 ? 0.25f : 0.75f;
+                    const float a00 = lerpf(c000, c100, fx), a10 = lerpf(c010, c110, fx);
+                    const float a01 = lerpf(c001, c101, fx), a11 = lerpf(c011, c111, fx);
+                    const float b0 = lerpf(a00, a10, fy), b1 = lerpf(a01, a11, fy);
+                    uf[c * Nf + (unsigned)((z * fd.ny + y) * fd.nx + x)] = 2.f * lerpf(b0, b1, fz);
+                }
+            }
+        }
     }
 }
 
@@ -77,8 +89,8 @@ int launch_restrict(const Dims& fd, const float* in, float* out, cudaStream_t st
 }
 
 int launch_prolong(const Dims& cd, const float* uc, const Dims& fd, float* uf, cudaStream_t st) {
-    const dim3 block(128, 2);
-    const dim3 grid((fd.nx + 127) / 128, (fd.ny + 1) / 2, fd.nz);
+    const dim3 block(64, 4);
+    const dim3 grid((cd.nx + 1 + 63) / 64, (cd.ny + 1 + 3) / 4, cd.nz + 1);  // cells: i, j, k in [-1, n_c - 1]
     k_prolong<<<grid, block, 0, st>>>(uc, uf, cd, fd);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }

@@ -6,7 +6,7 @@
 For every size: the fused warp+force+update entry point for all six variants, the Gaussian
 smoothing at sigma 1.0 and 2.0 (3 components), restrict and prolong.  Inputs are the seeded blob
 phantom and a random smooth field with max |u| = 8 voxels (phantoms.sweep_inputs).  Reported per
-kernel: median CUDA-event time of `reps` launches after 3 warm-ups, effective GB/s = algorithmic
+kernel: median over `reps` samples of 10 back-to-back launches (CUDA events) after 3 warm-ups, effective GB/s = algorithmic
 bytes (DESIGN.md byte table) / time, and % of the measured HBM peak.  The same command with
 --reps 3 is what the ncu captures under profiles/ run.
 """
@@ -34,7 +34,9 @@ def hbm_peak():
         return 6650.0, "fallback"
 
 
-def median_ms(torch, stream, fn, reps):
+def median_ms(torch, stream, fn, reps, inner=10):
+    """Median over `reps` samples of (CUDA-event time of `inner` back-to-back launches) / inner: the
+    queue stays full, so the host's launch latency is not in the number."""
     for _ in range(3):
         fn()
     torch.cuda.synchronize()
@@ -42,10 +44,11 @@ def median_ms(torch, stream, fn, reps):
     for _ in range(reps):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
-        fn()
+        for _ in range(inner):
+            fn()
         e1.record(stream)
         e1.synchronize()
-        times.append(e0.elapsed_time(e1))
+        times.append(e0.elapsed_time(e1) / inner)
     return float(np.median(times))
 
 
