@@ -44,6 +44,7 @@ struct SmoothArgs {
     int zc_override;   // > 0: planes per CTA of the fused kernel (tuning)
     int no_tma;        // 1 = skip the TMA kernel (use the LDG-fed fused kernel)
     int tune;          // kernel-configuration selector (tuning experiments; 0 = default)
+    int ascending;     // 1 = the fused kernel marches z upwards (default 0: downwards, see smooth_tma.cu)
 };
 int launch_smooth(const SmoothArgs& a, cudaStream_t stream);
 

@@ -16,6 +16,9 @@
 // clamped when the shared-memory addresses are formed.
 // HBM sees every element once in and once out (8 B / element); the paper's design was one
 // kernel per axis through shared memory (L175), i.e. 24 B / element.
+// The march runs DOWN the z axis by default (`rev`): the force kernels march up, so the planes they
+// wrote last are read first while they are still in L2, and the planes written last here are the
+// ones the next force kernel reads first.  The taps are symmetric: the result is bit-identical.
 #include <cstdio>
 #include <cstdlib>
 
@@ -65,7 +68,7 @@ struct Cfg {
 template <int R, int K, int RG, int STAGES, int MINB>
 __global__ void __launch_bounds__(32 * (RG + 1), MINB)
     k_smooth_tma(const __grid_constant__ CUtensorMap tmap, float* __restrict__ out, const Dims d, const int zc,
-                 const int tiles_x, const Taps t, const int* __restrict__ skip) {
+                 const int tiles_x, const Taps t, const int* __restrict__ skip, const int rev) {
     using C = Cfg<R, K, RG, STAGES>;
     constexpr int NH = C::NH, L = C::L, GX = C::GX, GW = C::GW, TY = C::TY, BOXW = C::BOXW;
     extern __shared__ __align__(1024) unsigned char smem[];
@@ -116,7 +119,7 @@ __global__ void __launch_bounds__(32 * (RG + 1), MINB)
     const bool issuer = halo_warp && lane == 0;
     auto issue = [&](int p) {  // plane p of the march -> stage p % STAGES
         const int s = p % STAGES;
-        const int z = min(max(z_start - R + p, 0), d.nz - 1);
+        const int z = min(max(rev ? z_start + nplanes - 1 + R - p : z_start - R + p, 0), d.nz - 1);
         mbar_expect_tx(&full[s], (uint32_t)(C::ROWS * BOXW * 4));
         tma::load_4d(smem + s * C::STAGE_BYTES, &tmap, &full[s], x0 - 4 * NH, y0 - R, z, comp);
     };
@@ -204,7 +207,7 @@ __global__ void __launch_bounds__(32 * (RG + 1), MINB)
                     }
                     // ---- z pass: register ring, packed f32x2 ----
                     if (p >= 2 * R) {
-                        float* orow = dst + (size_t)(z_start + p - 2 * R) * plane;
+                        float* orow = dst + (size_t)(rev ? z_start + nplanes - 1 - (p - 2 * R) : z_start + p - 2 * R) * plane;
 #pragma unroll
                         for (int j = 0; j < K; ++j) {
                             const F4& c = ring[(s - R + L) % L][j];
@@ -260,7 +263,7 @@ int launch_cfg(const SmoothArgs& a, int zc, cudaStream_t st) {
     Taps t;
     for (int k = 0; k < 8; ++k) t.w[k] = k <= a.R ? a.w[k] : 0.f;
     const dim3 grid(tiles_x * tiles_y, chunks, a.ncomp);
-    k_smooth_tma<R, K, RG, STAGES, MINB><<<grid, C::THREADS, C::SMEM, st>>>(map, a.out, d, zc, tiles_x, t, a.skip);
+    k_smooth_tma<R, K, RG, STAGES, MINB><<<grid, C::THREADS, C::SMEM, st>>>(map, a.out, d, zc, tiles_x, t, a.skip, a.ascending ? 0 : 1);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
