@@ -415,3 +415,55 @@ void oracle_ic_error(const float* uf, const float* ub, const int dims[3], double
     *mean = sum / (double)N;
     *max = mx;
 }
+
+/* Correlation coefficient between the deformed moving image and the static image (PAPER.md L234,
+ * Sec. 3.3: the "commonly used" similarity measure the paper compares its relative norm with):
+ *   CC = sum (a - mean a)(b - mean b) / sqrt( sum (a - mean a)^2  sum (b - mean b)^2 ),
+ * a = warp(M,u), b = S (variant 5: b = warp(S,ub)).  Two passes (means first), all in double.
+ * Returns 0 when either image is constant. */
+double oracle_cc(int variant, const int dims[3], const float* S, const float* M, const float* u,
+                 const float* ub) {
+    const size_t N = nvox(dims);
+    const int ic = variant == ORACLE_INVERSE_CONSISTENT;
+    float* Mw = (float*)malloc(N * sizeof(float));
+    float* Sw = ic ? (float*)malloc(N * sizeof(float)) : NULL;
+    oracle_warp(M, u, dims, Mw);
+    if (ic) oracle_warp(S, ub, dims, Sw);
+    const float* b = ic ? Sw : S;
+    double ma = 0.0, mb = 0.0;
+    for (size_t i = 0; i < N; ++i) {
+        ma += (double)Mw[i];
+        mb += (double)b[i];
+    }
+    ma /= (double)N;
+    mb /= (double)N;
+    double sab = 0.0, saa = 0.0, sbb = 0.0;
+    for (size_t i = 0; i < N; ++i) {
+        const double da = (double)Mw[i] - ma, db = (double)b[i] - mb;
+        sab += da * db;
+        saa += da * da;
+        sbb += db * db;
+    }
+    free(Mw);
+    free(Sw);
+    return (saa > 0.0 && sbb > 0.0) ? sab / sqrt(saa * sbb) : 0.0;
+}
+
+/* Landmark-style evaluation (Sec. 3.2: "three-dimensional Euclidean distance" at
+ * feature points): for each point p_i (voxel coordinates, any real position) sample the field
+ * trilinearly (clamped, O2) and return  err_i = | (u(p_i) - expect_i) * spacing |_2  in mm.
+ * points, expect: [n][3] (x, y, z); err: [n]. */
+void oracle_point_error(const float* u, const int dims[3], const double spacing[3], int n,
+                        const float* points, const float* expect, double* err) {
+    const size_t N = nvox(dims);
+    for (int i = 0; i < n; ++i) {
+        double e2 = 0.0;
+        for (int c = 0; c < 3; ++c) {
+            const double v = sample_trilinear(u + c * N, dims, (double)points[3 * i], (double)points[3 * i + 1],
+                                              (double)points[3 * i + 2]);
+            const double d = (v - (double)expect[3 * i + c]) * spacing[c];
+            e2 += d * d;
+        }
+        err[i] = sqrt(e2);
+    }
+}

@@ -82,6 +82,15 @@ double oracle_final_ssd(int variant, const int dims[3], const float* S, const fl
 /* BASELINE.json config 4: e(x) = | u_f(x) + u_b(x + u_f(x)) |, u_b sampled trilinearly, clamped. */
 void oracle_ic_error(const float* uf, const float* ub, const int dims[3], double* mean, double* max);
 
+/* Correlation coefficient of warp(M,u) and S (variant 5: warp(S,ub)). */
+double oracle_cc(int variant, const int dims[3], const float* S, const float* M, const float* u,
+                 const float* ub);
+
+/* 3D Euclidean error in mm of the field sampled at n points against expected
+ * displacements; points / expect: [n][3] in voxels, err: [n]. */
+void oracle_point_error(const float* u, const int dims[3], const double spacing[3], int n,
+                        const float* points, const float* expect, double* err);
+
 #ifdef __cplusplus
 }
 #endif

@@ -38,6 +38,7 @@ def lib():
     if _lib is None:
         _lib = ctypes.CDLL(build())
         _lib.oracle_final_ssd.restype = ctypes.c_double
+        _lib.oracle_cc.restype = ctypes.c_double
         _lib.oracle_gauss_taps.restype = ctypes.c_int
         _lib.oracle_register.restype = ctypes.c_int
     return _lib
@@ -164,6 +165,21 @@ def ic_error(uf, ub):
     mean, mx = ctypes.c_double(), ctypes.c_double()
     lib().oracle_ic_error(_ptr(uf), _ptr(ub), _dims_of(uf.shape), ctypes.byref(mean), ctypes.byref(mx))
     return mean.value, mx.value
+
+
+def cc(variant, S, M, u, ub=None):
+    S, M, u = _f32(S), _f32(M), _f32(u)
+    ub = _f32(ub) if ub is not None else None
+    return float(lib().oracle_cc(ctypes.c_int(variant), _dims_of(S.shape), _ptr(S), _ptr(M), _ptr(u), _ptr(ub)))
+
+
+def point_error(u, spacing, points, expect):
+    u, points, expect = _f32(u), _f32(points), _f32(expect)
+    n = points.shape[0]
+    err = np.empty(n, dtype=np.float64)
+    sp = (ctypes.c_double * 3)(*[float(v) for v in spacing])
+    lib().oracle_point_error(_ptr(u), _dims_of(u.shape), sp, ctypes.c_int(n), _ptr(points), _ptr(expect), _ptr(err))
+    return err
 
 
 if __name__ == "__main__":

@@ -422,3 +422,58 @@ def test_stopping_rule(oracle):  # O10
     assert early["iters_done"] == [n_stop + 1]
     again = oracle.register(0, 1.0, 1.0, S, M, [n_stop + 1])
     assert np.array_equal(early["u"], again["u"])
+
+
+def test_cc_pins(oracle):
+    """Correlation coefficient: affine invariance, sign, library value."""
+    rng = np.random.default_rng(31)
+    S = (rng.standard_normal((6, 7, 9)) * 100).astype(np.float32)
+    Mx = (rng.standard_normal((6, 7, 9)) * 50 + 20).astype(np.float32)
+    zero = np.zeros((3,) + S.shape, np.float32)
+    assert oracle.cc(0, S, S, zero) == pytest.approx(1.0, abs=1e-12)
+    assert oracle.cc(0, S, (3.0 * S + 7.0).astype(np.float32), zero) == pytest.approx(1.0, abs=1e-6)   # CC(aX+b, X) = 1
+    assert oracle.cc(0, S, (-0.5 * S + 2.0).astype(np.float32), zero) == pytest.approx(-1.0, abs=1e-6)
+    assert oracle.cc(0, S, np.full_like(S, 4.0), zero) == 0.0                                      # constant image
+    lib_value = np.corrcoef(S.ravel().astype(np.float64), Mx.ravel().astype(np.float64))[0, 1]
+    assert oracle.cc(0, S, Mx, zero) == pytest.approx(lib_value, rel=1e-12, abs=1e-14)
+    assert oracle.cc(0, S, Mx, zero) == pytest.approx(oracle.cc(0, Mx, S, zero), abs=1e-14)        # symmetric
+    # an integer shift of the field shifts the moving image before it is correlated
+    u = np.zeros((3,) + S.shape, np.float32)
+    u[0] = 1.0
+    shifted = S.copy()
+    shifted[:, :, 1:] = S[:, :, :-1]
+    shifted[:, :, 0] = S[:, :, 0]           # M(x + 1) = S(x) inside, clamped at the face
+    a = oracle.warp(shifted, u).ravel().astype(np.float64)
+    assert oracle.cc(0, S, shifted, u) == pytest.approx(np.corrcoef(a, S.ravel().astype(np.float64))[0, 1], rel=1e-12)
+    # variant 5 correlates the two warped images
+    ub = np.zeros_like(u)
+    ub[1] = -1.0
+    b = oracle.warp(S, ub).ravel().astype(np.float64)
+    assert oracle.cc(5, S, shifted, u, ub) == pytest.approx(np.corrcoef(a, b)[0, 1], rel=1e-12)
+
+
+def test_point_error_pins(oracle):
+    """3D Euclidean error at points: closed forms on a linear field, spacing, clamp."""
+    nz, ny, nx = 5, 6, 8
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    u = np.stack([0.5 * x + 1.0, -0.25 * y, 2.0 + 0 * z]).astype(np.float32)   # trilinear reproduces linear fields
+    pts = np.array([[1.5, 2.25, 3.0], [0.0, 0.0, 0.0], [6.75, 4.5, 1.25]], np.float32)
+    exact = np.stack([0.5 * pts[:, 0] + 1.0, -0.25 * pts[:, 1], np.full(3, 2.0)], axis=1)
+    sp = (0.97, 0.97, 2.5)
+    assert np.allclose(oracle.point_error(u, sp, pts, exact.astype(np.float32)), 0.0, atol=1e-6)
+    off = exact + np.array([[3.0, 0.0, 0.0], [0.0, -4.0, 0.0], [1.0, 2.0, 2.0]])
+    want = np.sqrt((np.array([[3.0, 0, 0], [0, 4.0, 0], [1.0, 2.0, 2.0]]) * np.array(sp)) ** 2).sum(axis=1) ** 1.0
+    want = np.linalg.norm(np.array([[3.0, 0, 0], [0, 4.0, 0], [1.0, 2.0, 2.0]]) * np.array(sp), axis=1)
+    assert np.allclose(oracle.point_error(u, sp, pts, off.astype(np.float32)), want, rtol=1e-6)
+    # outside the volume the sample clamps to the face value
+    far = np.array([[-5.0, 100.0, 2.0]], np.float32)
+    face = np.array([[0.5 * 0 + 1.0, -0.25 * (ny - 1), 2.0]], np.float32)
+    assert np.allclose(oracle.point_error(u, (1, 1, 1), far, face), 0.0, atol=1e-6)
+    # against the library resampler on a random field
+    rng = np.random.default_rng(5)
+    ur = rng.standard_normal((3, nz, ny, nx)).astype(np.float32)
+    p = (rng.random((20, 3)) * np.array([nx - 1, ny - 1, nz - 1])).astype(np.float32)
+    coords = [p[:, 2].astype(np.float64), p[:, 1].astype(np.float64), p[:, 0].astype(np.float64)]
+    lib_u = np.stack([ndimage.map_coordinates(ur[c].astype(np.float64), coords, order=1, mode="nearest") for c in range(3)], axis=1)
+    err = oracle.point_error(ur, (1, 1, 1), p, np.zeros((20, 3), np.float32))
+    assert np.allclose(err, np.linalg.norm(lib_u, axis=1), rtol=1e-9, atol=1e-12)
