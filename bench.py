@@ -196,7 +196,7 @@ def main():
     replicas.init("nccl")
     N = DIMS[0] * DIMS[1] * DIMS[2]
 
-    S, M, _ = phantoms.lung_pair(DIMS, replicas.replica_seed(202, rank))
+    S, M, _d_known = phantoms.lung_pair(DIMS, replicas.replica_seed(202, rank))
     dS, dM = torch.from_numpy(S).to(device), torch.from_numpy(M).to(device)
     du = torch.zeros((3,) + S.shape, dtype=torch.float32, device=device)
     eng = B.Demons(DIMS, SPACING, B.PASSIVE, 1.0, SIGMA, levels=1, device=device)
@@ -211,6 +211,31 @@ def main():
     units = args.steps * sum(ITERS) * N
     agg = replicas.aggregate(units, secs, device)
     final_u_absmax = float(du.abs().max())
+    # BASELINE.json config 2: 3D error at 1,000 seeded interior points against the known field
+    # (PAPER.md L222 protocol) and the correlation coefficient (L234), through the C ABI
+    evaluation = None
+    if rank == 0:
+        pts = phantoms.eval_points(DIMS, np.random.default_rng(2020), 1000)
+        truth = phantoms.true_inverse_at(_d_known, pts).astype(np.float32)
+        dpts = torch.from_numpy(pts.astype(np.float32)).to(device)
+        dtruth = torch.from_numpy(truth).to(device)
+        derr = torch.zeros(1000, dtype=torch.float64, device=device)
+        dcc = torch.zeros(1, dtype=torch.float64, device=device)
+        B.demons_point_error(eng.ctx, DIMS, du, 1000, dpts, dtruth, derr, stream)
+        B.demons_cc(eng.ctx, DIMS, dS, dM, du, None, dcc, stream)
+        torch.cuda.synchronize()
+        err_after, cc_after = derr.cpu().numpy().copy(), float(dcc[0])
+        zero = torch.zeros_like(du)
+        B.demons_point_error(eng.ctx, DIMS, zero, 1000, dpts, dtruth, derr, stream)
+        B.demons_cc(eng.ctx, DIMS, dS, dM, zero, None, dcc, stream)
+        torch.cuda.synchronize()
+        err_before, cc_before = derr.cpu().numpy(), float(dcc[0])
+        del zero
+        evaluation = {"points": 1000, "err_mm_mean_before": float(err_before.mean()), "err_mm_sd_before": float(err_before.std()),
+                      "err_mm_mean_after": float(err_after.mean()), "err_mm_sd_after": float(err_after.std()),
+                      "cc_before": cc_before, "cc_after": cc_after,
+                      "note": "single-scale passive demons cannot capture the 12-voxel motion of config 2 in 300 "
+                              "iterations (SURVEY.md 8d); parity and throughput are what this bench grades"}
 
     # ---- end to end through the C ABI with pinned host buffers ----
     hS, hM = torch.from_numpy(S).pin_memory(), torch.from_numpy(M).pin_memory()
@@ -285,10 +310,11 @@ def main():
         "gpu_launches": int(launches),
         "roofline": roofline,
         "final_u_absmax_voxel": final_u_absmax,
+        "evaluation": evaluation,
     }
 
     if rank == 0 and world == 1 and not args.no_extras:
-        line["variants"] = bench_variants(torch, B, phantoms, replicas, S, M, device, stream)
+        line["variants"] = bench_variants(torch, B, phantoms, replicas, S, M, _d_known, device, stream)
         sample_iters = 6
         t = oracle_sample(S, M, sample_iters)
         line["cpu_baseline"] = {"value": sample_iters * N / t / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
@@ -302,13 +328,17 @@ def main():
         dist.destroy_process_group()
 
 
-def bench_variants(torch, B, phantoms, replicas, S, M, device, stream):
+def bench_variants(torch, B, phantoms, replicas, S, M, d_known, device, stream):
     """BASELINE.json configs 3-4: every variant, three-level pyramid, 100 iterations per level."""
     out = {}
     iters = [100, 100, 100]
     cases = [(0, 1.0, "passive"), (1, 1.0, "evolved_passive"), (2, 1.0, "active"), (3, 1.0, "double"),
              (4, 0.4, "adjusted_double_a0.4"), (5, 1.0, "inverse_consistent")]
     dS, dM = torch.from_numpy(S).to(device), torch.from_numpy(M).to(device)
+    pts = phantoms.eval_points(DIMS, np.random.default_rng(2020), 1000)
+    dpts = torch.from_numpy(pts.astype(np.float32)).to(device)
+    dtruth = torch.from_numpy(phantoms.true_inverse_at(d_known, pts).astype(np.float32)).to(device)
+    derr = torch.zeros(1000, dtype=torch.float64, device=device)
     for variant, alpha, name in cases:
         eng = B.Demons(DIMS, SPACING, variant, alpha, SIGMA, levels=3, device=device)
         du = torch.zeros((3,) + S.shape, dtype=torch.float32, device=device)
@@ -318,8 +348,12 @@ def bench_variants(torch, B, phantoms, replicas, S, M, device, stream):
         for l in range(3):
             d = B.demons_level_dims(eng.ctx, l)
             voxel_iters += d[0] * d[1] * d[2] * 100
+        B.demons_point_error(eng.ctx, DIMS, du, 1000, dpts, dtruth, derr, stream)
+        torch.cuda.synchronize()
+        e = derr.cpu().numpy()
         out[name] = {"ms_per_registration": 1e3 * secs / 3, "gvoxel_iter_per_s": 3 * voxel_iters / secs / 1e9,
-                     "launches_per_registration": launches // 3}
+                     "launches_per_registration": launches // 3,
+                     "err_mm_mean": float(e.mean()), "err_mm_sd": float(e.std())}
         eng.close()
     return out
 

@@ -162,6 +162,22 @@ int demons_ssd(demons_ctx* ctx, const int dims[3], const float* d_static, const 
 int demons_ic_error(demons_ctx* ctx, const int dims[3], const float* d_uf, const float* d_ub,
                     double* d_out, void* stream);
 
+/* demons_cc: correlation coefficient between the deformed moving image and the static image,
+ *   CC = sum (a - mean a)(b - mean b) / sqrt( sum (a - mean a)^2 sum (b - mean b)^2 ),
+ * a = warp(M,u), b = S (variant 5: b = warp(S,ub), d_ub NULL otherwise) -- the similarity measure
+ * PAPER.md L234 (Sec. 3.3) compares the relative-norm stopping rule with.  0 if either image is
+ * constant.  d_out: 1 double on the device. */
+int demons_cc(demons_ctx* ctx, const int dims[3], const float* d_static, const float* d_moving,
+              const float* d_u, const float* d_ub, double* d_out, void* stream);
+
+/* demons_point_error: the landmark evaluation of PAPER.md L222 (Sec. 3.2, "three-dimensional
+ * Euclidean distance").  d_points: [n][3] positions (x, y, z) in voxels of `dims`, any real value
+ * (clamped to the volume); d_expect: [n][3] expected displacement at those points in voxels;
+ * d_err: [n] doubles on the device = | (u(p_i) - expect_i) * spacing |_2 in mm, u sampled
+ * trilinearly, spacing = the context's.  n_points == 0 is a no-op. */
+int demons_point_error(demons_ctx* ctx, const int dims[3], const float* d_u, int n_points,
+                       const float* d_points, const float* d_expect, double* d_err, void* stream);
+
 /* Thread-local description of the last failure on this thread ("" if none). */
 const char* demons_last_error(void);
 

@@ -42,6 +42,8 @@ SIGNATURES = {
     "demons_prolong": (ctypes.c_int, [_vp, _c_int3, _vp, _c_int3, _vp, _vp]),
     "demons_ssd": (ctypes.c_int, [_vp, _c_int3, _vp, _vp, _vp, _vp, _vp, _vp]),
     "demons_ic_error": (ctypes.c_int, [_vp, _c_int3, _vp, _vp, _vp, _vp]),
+    "demons_cc": (ctypes.c_int, [_vp, _c_int3, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "demons_point_error": (ctypes.c_int, [_vp, _c_int3, _vp, ctypes.c_int, _vp, _vp, _vp, _vp]),
     "demons_last_error": (ctypes.c_char_p, []),
 }
 
@@ -187,6 +189,16 @@ def demons_ssd(ctx, dims, d_static, d_moving, d_u, d_ub, d_out, stream=None):
 
 def demons_ic_error(ctx, dims, d_uf, d_ub, d_out, stream=None):
     _check(lib().demons_ic_error(ctx, _int3(dims), _ptr(d_uf), _ptr(d_ub), _ptr(d_out), _stream(stream)))
+
+
+def demons_cc(ctx, dims, d_static, d_moving, d_u, d_ub, d_out, stream=None):
+    _check(lib().demons_cc(ctx, _int3(dims), _ptr(d_static), _ptr(d_moving), _ptr(d_u), _ptr(d_ub), _ptr(d_out),
+                           _stream(stream)))
+
+
+def demons_point_error(ctx, dims, d_u, n_points, d_points, d_expect, d_err, stream=None):
+    _check(lib().demons_point_error(ctx, _int3(dims), _ptr(d_u), int(n_points), _ptr(d_points), _ptr(d_expect),
+                                    _ptr(d_err), _stream(stream)))
 
 
 def demons_last_error():

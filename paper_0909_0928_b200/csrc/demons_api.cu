@@ -138,7 +138,7 @@ Partition make_partition(const demons_ctx* c, int levels) {
     int stride = force_partial_blocks(c->dims);
     if (stride < 148 * 8) stride = 148 * 8;
     p.partial_stride = stride;
-    p.partials = take(3 * (size_t)stride * sizeof(double));
+    p.partials = take(5 * (size_t)stride * sizeof(double));  // 3 metrics per force block; 5 sums per block of demons_cc
     p.stats = take((size_t)DEMONS_MAX_STATS_ROWS * 3 * sizeof(double));
     p.Mw = take(N * 4);
     p.Sw = ic ? take(N * 4) : 0;
@@ -756,6 +756,40 @@ int demons_ic_error(demons_ctx* c, const int dims[3], const float* d_uf, const f
                      &reinterpret_cast<Control*>(c->ws + p.control)->ticket, p.partial_stride};
     if (launch_ic_error(d, d_uf, d_ub, d_out, rs, static_cast<cudaStream_t>(stream)) < 0)
         return fail(DEMONS_E_CUDA, "ic_error launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    c->launches += 1;
+    return DEMONS_OK;
+}
+
+int demons_cc(demons_ctx* c, const int dims[3], const float* d_static, const float* d_moving, const float* d_u,
+              const float* d_ub, double* d_out, void* stream) {
+    if (!c) return fail(DEMONS_E_ARG, "ctx is NULL");
+    Dims d;
+    int rc = check_call_dims(c, dims, &d);
+    if (rc != DEMONS_OK) return rc;
+    if (!d_static || !d_moving || !d_u || !d_out) return fail(DEMONS_E_ARG, "NULL pointer");
+    if (is_ic(c) && !d_ub) return fail(DEMONS_E_ARG, "variant 5 needs u_back");
+    if (!is_ic(c) && d_ub) return fail(DEMONS_E_ARG, "u_back must be NULL unless variant 5");
+    rc = check_ws(c, 1);
+    if (rc != DEMONS_OK) return rc;
+    const Partition p = make_partition(c, 1);
+    ReduceScratch rs{reinterpret_cast<double*>(c->ws + p.partials),
+                     &reinterpret_cast<Control*>(c->ws + p.control)->ticket, p.partial_stride};
+    if (launch_cc(d, d_static, d_moving, d_u, d_ub, d_out, rs, static_cast<cudaStream_t>(stream)) < 0)
+        return fail(DEMONS_E_CUDA, "cc launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    c->launches += 1;
+    return DEMONS_OK;
+}
+
+int demons_point_error(demons_ctx* c, const int dims[3], const float* d_u, int n_points, const float* d_points,
+                       const float* d_expect, double* d_err, void* stream) {
+    if (!c) return fail(DEMONS_E_ARG, "ctx is NULL");
+    if (!dims_ok(dims)) return fail(DEMONS_E_ARG, "bad dims");
+    if (n_points < 0) return fail(DEMONS_E_ARG, "negative point count");
+    if (n_points == 0) return DEMONS_OK;
+    if (!d_u || !d_points || !d_expect || !d_err) return fail(DEMONS_E_ARG, "NULL pointer");
+    const Dims d{dims[0], dims[1], dims[2]};
+    if (launch_point_error(d, c->spacing, d_u, n_points, d_points, d_expect, d_err, static_cast<cudaStream_t>(stream)) < 0)
+        return fail(DEMONS_E_CUDA, "point_error launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     c->launches += 1;
     return DEMONS_OK;
 }

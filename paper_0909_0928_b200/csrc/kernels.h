@@ -60,5 +60,9 @@ int launch_ssd(const Dims& d, const float* S, const float* M, const float* u, co
                double* out, const ReduceScratch& rs, cudaStream_t stream);
 int launch_ic_error(const Dims& d, const float* uf, const float* ub, double* out,
                     const ReduceScratch& rs, cudaStream_t stream);
+int launch_cc(const Dims& d, const float* S, const float* M, const float* u, const float* ub, double* out,
+              const ReduceScratch& rs, cudaStream_t stream);
+int launch_point_error(const Dims& d, const float spacing[3], const float* u, int n, const float* points,
+                       const float* expect, double* err, cudaStream_t stream);
 
 }  // namespace demons

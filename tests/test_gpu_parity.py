@@ -437,3 +437,47 @@ def test_full_size_registration_prefix_matches_oracle(torch_cuda, B, oracle, lun
     ref = oracle.register(0, 1.0, 1.0, S, M, iters)
     res = run_register(torch_cuda, B, 0, S, M, iters)
     check_registration(res, ref, "config 2 prefix")
+
+
+@pytest.mark.parametrize("variant", [0, 5])
+def test_cc_matches_oracle(torch_cuda, B, P, oracle, variant):
+    """Correlation coefficient: one-pass raw sums on the GPU, two-pass oracle."""
+    torch = torch_cuda
+    dims = (66, 35, 19)
+    S, M, u, ub = make_case(P, dims, seed=11)
+    S = (S - 500.0).astype(np.float32)   # a large mean makes the one-pass cancellation visible if it is wrong
+    M = (M - 500.0).astype(np.float32)
+    ic = variant == 5
+    eng = B.Demons(dims, variant=variant)
+    out = torch.zeros(1, dtype=torch.float64, device="cuda:0")
+    B.demons_cc(eng.ctx, dims, dev(torch, S), dev(torch, M), dev(torch, u), dev(torch, ub) if ic else None, out)
+    torch.cuda.synchronize()
+    ref = oracle.cc(variant, S, M, u, ub if ic else None)
+    assert abs(float(out[0]) - ref) <= 1e-6
+    # constant image -> 0 by definition
+    B.demons_cc(eng.ctx, dims, dev(torch, np.full_like(S, 7.0)), dev(torch, M), dev(torch, u),
+                dev(torch, ub) if ic else None, out)
+    torch.cuda.synchronize()
+    if not ic:
+        assert float(out[0]) == 0.0
+    eng.close()
+
+
+def test_point_error_matches_oracle(torch_cuda, B, P, oracle):
+    """Landmark-style evaluation: 1,000 points, also outside the volume."""
+    torch = torch_cuda
+    dims = (40, 24, 12)
+    spacing = (0.97, 0.97, 2.5)
+    rng = np.random.default_rng(3)
+    u = P.bump_field(dims, rng, 6, (3.0, 9.0), 3.0, centre_frac=1.0)
+    pts = (rng.random((1000, 3)) * (np.array(dims) + 4.0) - 2.0).astype(np.float32)
+    pts[:50] = np.round(pts[:50])           # integer positions as well
+    expect = rng.standard_normal((1000, 3)).astype(np.float32)
+    ref = oracle.point_error(u, spacing, pts, expect)
+    eng = B.Demons(dims, spacing=spacing)
+    err = torch.zeros(1000, dtype=torch.float64, device="cuda:0")
+    B.demons_point_error(eng.ctx, dims, dev(torch, u), 1000, dev(torch, pts), dev(torch, expect), err)
+    torch.cuda.synchronize()
+    assert_close(err.cpu().numpy(), ref, "point error (mm)")
+    B.demons_point_error(eng.ctx, dims, dev(torch, u), 0, None, None, None)   # empty input is a no-op
+    eng.close()
