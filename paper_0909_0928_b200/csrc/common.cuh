@@ -100,29 +100,36 @@ __device__ __forceinline__ void clamp_cell_axis(int& i, float& f, int n) {
     i = min(max(i, 0), n - 2);
 }
 
-// Cells of NV voxels (xs[j], y, z) of one lane.  The clamp arithmetic is skipped when no lane of
-// the warp needs it (warp-uniform test; only pure ALU code sits under the branch).
+// Cells of NV voxels (xs[j], y, z) of one lane.  The clamp arithmetic of an axis is skipped when no
+// lane of the warp needs it (warp-uniform tests; only pure ALU code sits under the branches).
 template <int NV>
 __device__ __forceinline__ void make_cells(const Dims& d, const int (&xs)[NV], int y, int z, const float (&ux)[NV],
                                            const float (&uy)[NV], const float (&uz)[NV], unsigned (&o)[NV],
                                            float (&fx)[NV], float (&fy)[NV], float (&fz)[NV]) {
     int ix[NV], iy[NV], iz[NV];
-    bool inside = true;
+    bool inx = true, iny = true, inz = true;
 #pragma unroll
     for (int j = 0; j < NV; ++j) {
         ix[j] = floor_split(xs[j], ux[j], fx[j]);
         iy[j] = floor_split(y, uy[j], fy[j]);
         iz[j] = floor_split(z, uz[j], fz[j]);
-        inside = inside && (unsigned)ix[j] < (unsigned)(d.nx - 1) && (unsigned)iy[j] < (unsigned)(d.ny - 1) &&
-                 (unsigned)iz[j] < (unsigned)(d.nz - 1);
+        inx = inx && (unsigned)ix[j] < (unsigned)(d.nx - 1);
+        iny = iny && (unsigned)iy[j] < (unsigned)(d.ny - 1);
+        inz = inz && (unsigned)iz[j] < (unsigned)(d.nz - 1);
     }
-    if (!__all_sync(__activemask(), inside)) {
+    // one vote per axis: a warp that spans a row end nearly always needs the x clamp, rarely the others
+    const unsigned mask = __activemask();
+    if (!__all_sync(mask, inx)) {
 #pragma unroll
-        for (int j = 0; j < NV; ++j) {
-            clamp_cell_axis(ix[j], fx[j], d.nx);
-            clamp_cell_axis(iy[j], fy[j], d.ny);
-            clamp_cell_axis(iz[j], fz[j], d.nz);
-        }
+        for (int j = 0; j < NV; ++j) clamp_cell_axis(ix[j], fx[j], d.nx);
+    }
+    if (!__all_sync(mask, iny)) {
+#pragma unroll
+        for (int j = 0; j < NV; ++j) clamp_cell_axis(iy[j], fy[j], d.ny);
+    }
+    if (!__all_sync(mask, inz)) {
+#pragma unroll
+        for (int j = 0; j < NV; ++j) clamp_cell_axis(iz[j], fz[j], d.nz);
     }
 #pragma unroll
     for (int j = 0; j < NV; ++j) o[j] = (unsigned)((iz[j] * d.ny + iy[j]) * d.nx + ix[j]);

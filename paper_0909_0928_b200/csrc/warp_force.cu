@@ -662,15 +662,18 @@ int launch_lc(const ForceArgs& a, const KParams& p0, bool vec4, cudaStream_t st)
 template <bool TEX>
 int launch_lc_x(const ForceArgs& a, const KParams& p, bool vec4, cudaStream_t st) {
     int xpt = a.d.nx <= 32 ? 1 : a.d.nx <= 64 ? 2 : 4;
-    if (a.variant == 1 && xpt > 2) xpt = 2;  // two stencils: 4 voxels per lane spill at 128 registers (84 vs 73 us)
+    // Evolved passive (two stencils): 2 voxels per lane at 128 registers -- 4 voxels spill (84 us), 2 voxels
+    // at 80 registers spill too (80 us), 2 voxels at 128 registers do not (65 us, 256x256x100).
+    const bool two = a.variant == 1;
+    if (two && xpt > 2) xpt = 2;
     if ((a.tune >> 4) & 0xF) xpt = (a.tune >> 4) & 0xF;  // tuning experiments
     if (a.d.nx % (32 * xpt) == 0) {
         if (xpt == 1) return launch_lc<1, true, TEX, 3>(a, p, vec4, st);
-        if (xpt == 2) return launch_lc<2, true, TEX, 3>(a, p, vec4, st);
+        if (xpt == 2) return two ? launch_lc<2, true, TEX, 2>(a, p, vec4, st) : launch_lc<2, true, TEX, 3>(a, p, vec4, st);
         return launch_lc<4, true, TEX, 2>(a, p, vec4, st);
     }
     if (xpt == 1) return launch_lc<1, false, TEX, 3>(a, p, vec4, st);
-    if (xpt == 2) return launch_lc<2, false, TEX, 3>(a, p, vec4, st);
+    if (xpt == 2) return two ? launch_lc<2, false, TEX, 2>(a, p, vec4, st) : launch_lc<2, false, TEX, 3>(a, p, vec4, st);
     return launch_lc<4, false, TEX, 2>(a, p, vec4, st);
 }
 
