@@ -98,7 +98,9 @@ int demons_get_profile(const demons_ctx* ctx, double h_ms[4], long long h_launch
  * option only -- fails parity by design).  "generic_smooth" (default 0): always use
  * the three separable smoothing passes instead of the fused kernel.  "profile" (default 0): time
  * every kernel class with events inside demons_register (disables graphs, adds a final
- * synchronise; see demons_get_profile).  Unknown name -> DEMONS_E_ARG. */
+ * synchronise; see demons_get_profile).  Kernel-selection knobs used by the tuning experiments and the
+ * tests of the fallback paths, not part of the stable interface: "no_tma", "smooth_zc",
+ * "force_zper", "force_scalar", "tune".  Unknown name -> DEMONS_E_ARG. */
 int demons_set_option(demons_ctx* ctx, const char* name, int value);
 
 /* ---- full registration (PAPER.md L123-125 multi-scale, L145 stopping rule; O9/O10) ---------

@@ -508,7 +508,6 @@ int demons_create(demons_ctx** out, const int dims[3], const float spacing[3], i
     c->variant = variant;
     c->alpha = alpha;
     c->sigma = sigma;
-    if (const char* t = getenv("DEMONS_TUNE")) c->opt_tune = (int)strtol(t, nullptr, 0);  // tuning experiments
     *out = c;
     return DEMONS_OK;
 }
