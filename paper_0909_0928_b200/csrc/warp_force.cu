@@ -595,8 +595,8 @@ struct Shape {
 };
 
 template <typename K>
-Shape pick_shape(K kernel, int tiles_x, int ny, int nz, int override_zper) {
-    Shape best{BY, nz < ZPER ? ZPER : nz};
+Shape pick_shape(K kernel, int tiles_x, int ny, int nz, int override_zper, long long max_blocks) {
+    Shape best{BY, nz};
     long long best_cost = -1;
     for (int by = BY; by >= 4; --by) {
         int per_sm = 0;
@@ -607,15 +607,18 @@ Shape pick_shape(K kernel, int tiles_x, int ny, int nz, int override_zper) {
         const long long slots = (long long)sm_count() * per_sm, xy = (long long)tiles_x * ((ny + by - 1) / by);
         for (int chunks = 1; chunks <= nz; ++chunks) {
             int zper = (nz + chunks - 1) / chunks;
-            if (override_zper >= ZPER) zper = override_zper;
-            if (zper < ZPER) break;
+            if (override_zper >= 1) zper = override_zper;
             const long long blocks = xy * ((nz + zper - 1) / zper);
+            if (blocks > max_blocks) {  // more blocks than the metric partials have room for
+                if (override_zper >= 1) break;
+                continue;
+            }
             const long long cost = ((blocks + slots - 1) / slots) * by * per_sm * (zper + 2);
             if (best_cost < 0 || cost < best_cost) {
                 best_cost = cost;
                 best = Shape{by, zper};
             }
-            if (override_zper >= ZPER) break;
+            if (override_zper >= 1) break;
         }
     }
     return best;
@@ -628,7 +631,7 @@ int launch_lc(const ForceArgs& a, const KParams& p0, bool vec4, cudaStream_t st)
     const int tiles_x = (a.d.nx + 32 * XPT - 1) / (32 * XPT);
     KParams p = p0;
     auto run = [&](auto kernel) {
-        const Shape sh = pick_shape(kernel, tiles_x, a.d.ny, a.d.nz, a.zper);
+        const Shape sh = pick_shape(kernel, tiles_x, a.d.ny, a.d.nz, a.zper, force_partial_blocks(a.d));
         p.zper = sh.zper;
         const dim3 grid(tiles_x, (a.d.ny + sh.by - 1) / sh.by, (a.d.nz + sh.zper - 1) / sh.zper);
         kernel<<<grid, dim3(BX, sh.by), 0, st>>>(p);
@@ -680,9 +683,13 @@ int launch_lc_x(const ForceArgs& a, const KParams& p, bool vec4, cudaStream_t st
 }  // namespace
 
 int force_partial_blocks(const Dims& d) {
-    // the largest grid any force kernel uses: 32-voxel tiles, 4-row blocks (pick_shape), ZPER planes
-    const long long gx = (d.nx + BX - 1) / BX, gy = (d.ny + 3) / 4, gz = (d.nz + ZPER - 1) / ZPER;
-    return (int)(gx * gy * gz);
+    // the largest grid any force kernel uses: 32-voxel tiles, 4-row blocks and single planes (pick_shape takes
+    // short marches only on small volumes, where the launch would otherwise not fill the GPU), capped
+    const long long gx = (d.nx + BX - 1) / BX, gy = (d.ny + 3) / 4, gz = d.nz;
+    const long long scalar = gx * ((d.ny + BY - 1) / BY) * ((d.nz + ZPER - 1) / ZPER);  // k_force_fixed<VEC = 1>
+    long long n = gx * gy * gz;
+    if (n > 65536) n = 65536;
+    return (int)(n > scalar ? n : scalar);
 }
 
 int launch_warp_force(const ForceArgs& a, cudaStream_t st) {
