@@ -481,3 +481,32 @@ def test_point_error_matches_oracle(torch_cuda, B, P, oracle):
     assert_close(err.cpu().numpy(), ref, "point error (mm)")
     B.demons_point_error(eng.ctx, dims, dev(torch, u), 0, None, None, None)   # empty input is a no-op
     eng.close()
+
+
+@pytest.mark.parametrize("variant", [0, 3])
+def test_unaligned_buffers_take_the_scalar_paths(torch_cuda, B, P, oracle, variant):
+    """Buffers that start 4 bytes past a 16-byte boundary (no float4, no TMA): same results."""
+    torch = torch_cuda
+    dims = (64, 24, 10)
+    S, M, u, _ = make_case(P, dims, seed=21)
+
+    def shifted(a):  # a device tensor whose storage starts one float past an aligned allocation
+        flat = torch.empty(a.size + 1, dtype=torch.float32, device="cuda:0")
+        v = flat[1:].view(a.shape)
+        v.copy_(torch.from_numpy(np.ascontiguousarray(a)))
+        assert v.data_ptr() % 16 == 4
+        return v
+
+    ref_u, _, ref_m = oracle.warp_force(variant, 1.0, S, M, u, None)
+    eng = B.Demons(dims, variant=variant)
+    out = shifted(np.full_like(u, np.nan))
+    met = torch.zeros(3, dtype=torch.float64, device="cuda:0")
+    B.demons_warp_force(eng.ctx, dims, shifted(S), shifted(M), shifted(u), out, None, None, met)
+    torch.cuda.synchronize()
+    assert_close(out.cpu().numpy(), ref_u, f"unaligned u_out variant {variant}")
+    np.testing.assert_allclose(met.cpu().numpy(), ref_m, rtol=1e-5)
+    sm = shifted(np.full_like(u, np.nan))
+    B.demons_smooth(eng.ctx, dims, out, sm, 3, 1.0)
+    torch.cuda.synchronize()
+    assert_close(sm.cpu().numpy(), oracle.smooth(ref_u, 1.0), "unaligned smooth", atol=2e-4)
+    eng.close()
