@@ -6,16 +6,22 @@
 // lives in a register, grad S (and grad M0) are recomputed from a 6-point stencil whose re-reads
 // hit L1/L2, so the compulsory HBM traffic is u (12 B) + S (4 B) + M (4 B) in, u' (12 B) out.
 // Variants 2-5 need the gradient of the WARPED image (reading A8), i.e. the warped values of the
-// six neighbours: the warped image is materialised once (k_warp) and then stencilled
+// six neighbours: the warped image is materialised once (k_warp_lc) and then stencilled
 // (k_force_active) instead of gathering 7x per voxel, which would be instruction-bound.
+//
+// Two generations of kernels live here.  The fast path is the lane-consecutive family
+// (k_force_fixed_lc, k_warp_lc: one 2x2x2 cell offset per sample, no branch between the loads of a
+// plane).  The float4-per-lane kernels of the first design (k_force_fixed, k_warp) remain as the
+// path for volumes with an axis of length 1, where a 2x2x2 cell does not exist, and as the
+// reference point of the tuning experiments ("tune" = 2); k_force_active (no gathers) is float4.
 #include "kernels.h"
 
 namespace demons {
 
 namespace {
 
-constexpr int BX = 32;  // threads along x (each owns VEC consecutive voxels)
-constexpr int BY = 8;   // threads along y
+constexpr int BX = 32;  // threads along x
+constexpr int BY = 8;   // threads along y (the lane-consecutive kernels may be launched with 4..8 rows)
 
 __device__ __forceinline__ bool skip_pass(const MetricSink& s) {
     if (s.stop_force != nullptr && *reinterpret_cast<volatile int*>(s.stop_force) != 0) {
