@@ -48,7 +48,7 @@ __device__ __forceinline__ F4 ld_f4(const float* p) {
     return r;
 }
 
-template <int R, int K, int RG, int STAGES>
+template <int R, int K, int RG, int STAGES, int PAIR = 1>
 struct Cfg {
     static constexpr int NH = (R + 3) / 4;      // halo float4 groups per side
     static constexpr int L = 2 * R + 1;         // ring length
@@ -58,18 +58,21 @@ struct Cfg {
     static constexpr int ROWS = TY + 2 * R;     // rows per loaded plane
     static constexpr int BOXW = 4 * GW;         // floats per loaded row
     static constexpr int STAGE_BYTES = (ROWS * BOXW * 4 + 127) / 128 * 128;
-    static constexpr int XS_BYTES = 2 * TY * GW * 16;
+    static constexpr int LR = PAIR == 2 ? L + 1 : L;  // ring slots (even when planes go in pairs)
+    static constexpr int XS_BYTES = 2 * PAIR * TY * GW * 16;
     static constexpr int THREADS = 32 * (RG + 1);
     static constexpr int SMEM = STAGES * STAGE_BYTES + XS_BYTES + STAGES * 8 + 128;
     static_assert(2 * NH * RG <= 32, "halo jobs must fit one warp");
     static_assert(TY >= R, "tile must be at least R rows high");
+    static_assert(PAIR == 1 || (PAIR == 2 && STAGES % 2 == 0), "pairs need an even number of stages");
 };
 
-template <int R, int K, int RG, int STAGES, int MINB>
+template <int R, int K, int RG, int STAGES, int MINB, int PAIR>
 __global__ void __launch_bounds__(32 * (RG + 1), MINB)
     k_smooth_tma(const __grid_constant__ CUtensorMap tmap, float* __restrict__ out, const Dims d, const int zc,
                  const int tiles_x, const Taps t, const int* __restrict__ skip, const int rev) {
-    using C = Cfg<R, K, RG, STAGES>;
+    using C = Cfg<R, K, RG, STAGES, PAIR>;
+    constexpr int LR = C::LR;
     constexpr int NH = C::NH, L = C::L, GX = C::GX, GW = C::GW, TY = C::TY, BOXW = C::BOXW;
     extern __shared__ __align__(1024) unsigned char smem[];
     float4* xs = reinterpret_cast<float4*>(smem + STAGES * C::STAGE_BYTES);  // [2][TY][GW]
@@ -134,94 +137,127 @@ __global__ void __launch_bounds__(32 * (RG + 1), MINB)
     }
 
     float* dst = out + (size_t)comp * plane * d.nz + (size_t)(y0 + rg * K) * d.nx + xg;
-    F4 ring[L][K];
-    for (int pg = 0; pg < P; pg += L) {
+    F4 ring[LR][K];
+    auto xrow_of = [&](int p) { return xs + ((((p / PAIR) & 1) * PAIR + (p % PAIR)) * TY + rg * K) * GW; };
+    // ---- y pass of plane p: registers, packed f32x2; the y-smoothed float4s also go to the exchange buffer
+    auto ypass = [&](int p, F4 (&ys)[K], float4* xrow) {
+        const int stage = p % STAGES;
+        mbar_wait(&full[stage], (uint32_t)((p / STAGES) & 1));
+        const float* raw = reinterpret_cast<const float*>(smem + stage * C::STAGE_BYTES);
+        if (active) {
+            F4 v[K + 2 * R];
 #pragma unroll
-        for (int s = 0; s < L; ++s) {
-            const int p = pg + s;
-            if (p < P) {  // uniform over the CTA
-                const int stage = p % STAGES;
-                mbar_wait(&full[stage], (uint32_t)((p / STAGES) & 1));
-                const float* raw = reinterpret_cast<const float*>(smem + stage * C::STAGE_BYTES);
-                float4* xrow = xs + ((p & 1) * TY + rg * K) * GW;
-                F4 ys[K];
-                if (active) {
-                    // ---- y pass: registers, packed f32x2 ----
-                    F4 v[K + 2 * R];
+            for (int i = 0; i < K + 2 * R; ++i) v[i] = ld_f4(raw + rowoff[i]);
 #pragma unroll
-                    for (int i = 0; i < K + 2 * R; ++i) v[i] = ld_f4(raw + rowoff[i]);
+            for (int j = 0; j < K; ++j) {
+                float2 a = __fmul2_rn(w2[0], v[j + R].a), b = __fmul2_rn(w2[0], v[j + R].b);
 #pragma unroll
-                    for (int j = 0; j < K; ++j) {
-                        float2 a = __fmul2_rn(w2[0], v[j + R].a), b = __fmul2_rn(w2[0], v[j + R].b);
-#pragma unroll
-                        for (int k = 1; k <= R; ++k) {
-                            a = __ffma2_rn(w2[k], __fadd2_rn(v[j + R - k].a, v[j + R + k].a), a);
-                            b = __ffma2_rn(w2[k], __fadd2_rn(v[j + R - k].b, v[j + R + k].b), b);
-                        }
-                        if (outside) {  // rare: halo lanes / ragged tiles at the volume border
-                            if (xg < 0) {  // left of the volume: replicate x = 0
-                                a = make_float2(a.x, a.x);
-                                b = a;
-                            } else {  // right of the volume: replicate x = nx - 1
-                                b = make_float2(b.y, b.y);
-                                a = b;
-                            }
-                        }
-                        ys[j].a = a;
-                        ys[j].b = b;
-                        xrow[j * GW + g] = make_float4(a.x, a.y, b.x, b.y);
+                for (int k = 1; k <= R; ++k) {
+                    a = __ffma2_rn(w2[k], __fadd2_rn(v[j + R - k].a, v[j + R + k].a), a);
+                    b = __ffma2_rn(w2[k], __fadd2_rn(v[j + R - k].b, v[j + R + k].b), b);
+                }
+                if (outside) {  // rare: halo lanes / ragged tiles at the volume border
+                    if (xg < 0) {  // left of the volume: replicate x = 0
+                        a = make_float2(a.x, a.x);
+                        b = a;
+                    } else {  // right of the volume: replicate x = nx - 1
+                        b = make_float2(b.y, b.y);
+                        a = b;
                     }
                 }
-                __syncthreads();  // xs complete; every warp is done reading this raw stage
-                if (issuer && p + STAGES < P) issue(p + STAGES);
-                if (owner) {
-                    // ---- x pass: neighbours' float4s from the exchange buffer ----
+                ys[j].a = a;
+                ys[j].b = b;
+                xrow[j * GW + g] = make_float4(a.x, a.y, b.x, b.y);
+            }
+        }
+    };
+    // ---- x pass of plane p into ring slot sl (neighbours' float4s from the exchange buffer), then the
+    // z pass of the plane R behind it (register ring, packed f32x2) and its store
+    auto xzpass = [&](int p, int sl, const F4 (&ys)[K], const float4* xrow) {
 #pragma unroll
-                    for (int j = 0; j < K; ++j) {
-                        float a[4 * (2 * NH + 1)];
+        for (int j = 0; j < K; ++j) {
+            float a[4 * (2 * NH + 1)];
 #pragma unroll
-                        for (int h = 0; h < 2 * NH + 1; ++h) {
-                            if (h == NH) {
-                                a[4 * h + 0] = ys[j].a.x;
-                                a[4 * h + 1] = ys[j].a.y;
-                                a[4 * h + 2] = ys[j].b.x;
-                                a[4 * h + 3] = ys[j].b.y;
-                            } else {
-                                const float4 q = xrow[j * GW + g - NH + h];
-                                a[4 * h + 0] = q.x;
-                                a[4 * h + 1] = q.y;
-                                a[4 * h + 2] = q.z;
-                                a[4 * h + 3] = q.w;
-                            }
-                        }
-                        float o[4];
+            for (int h = 0; h < 2 * NH + 1; ++h) {
+                if (h == NH) {
+                    a[4 * h + 0] = ys[j].a.x;
+                    a[4 * h + 1] = ys[j].a.y;
+                    a[4 * h + 2] = ys[j].b.x;
+                    a[4 * h + 3] = ys[j].b.y;
+                } else {
+                    const float4 q = xrow[j * GW + g - NH + h];
+                    a[4 * h + 0] = q.x;
+                    a[4 * h + 1] = q.y;
+                    a[4 * h + 2] = q.z;
+                    a[4 * h + 3] = q.w;
+                }
+            }
+            float o[4];
 #pragma unroll
-                        for (int e = 0; e < 4; ++e) {
-                            float acc = t.w[0] * a[4 * NH + e];
+            for (int e = 0; e < 4; ++e) {
+                float acc = t.w[0] * a[4 * NH + e];
 #pragma unroll
-                            for (int k = 1; k <= R; ++k) acc = fmaf(t.w[k], a[4 * NH + e - k] + a[4 * NH + e + k], acc);
-                            o[e] = acc;
-                        }
-                        ring[s][j].a = make_float2(o[0], o[1]);
-                        ring[s][j].b = make_float2(o[2], o[3]);
+                for (int k = 1; k <= R; ++k) acc = fmaf(t.w[k], a[4 * NH + e - k] + a[4 * NH + e + k], acc);
+                o[e] = acc;
+            }
+            ring[sl][j].a = make_float2(o[0], o[1]);
+            ring[sl][j].b = make_float2(o[2], o[3]);
+        }
+        if (p >= 2 * R) {
+            float* orow = dst + (size_t)(rev ? z_start + nplanes - 1 - (p - 2 * R) : z_start + p - 2 * R) * plane;
+#pragma unroll
+            for (int j = 0; j < K; ++j) {
+                const F4& c = ring[(sl - R + LR) % LR][j];
+                float2 a = __fmul2_rn(w2[0], c.a), b = __fmul2_rn(w2[0], c.b);
+#pragma unroll
+                for (int k = 1; k <= R; ++k) {
+                    const F4& lo = ring[(sl - R - k + 2 * LR) % LR][j];
+                    const F4& hi = ring[(sl - R + k + LR) % LR][j];
+                    a = __ffma2_rn(w2[k], __fadd2_rn(lo.a, hi.a), a);
+                    b = __ffma2_rn(w2[k], __fadd2_rn(lo.b, hi.b), b);
+                }
+                if (y0 + rg * K + j < d.ny)
+                    *reinterpret_cast<float4*>(orow + (size_t)j * d.nx) = make_float4(a.x, a.y, b.x, b.y);
+            }
+        }
+    };
+    if constexpr (PAIR == 1) {
+        for (int pg = 0; pg < P; pg += LR) {
+#pragma unroll
+            for (int s = 0; s < LR; ++s) {
+                const int p = pg + s;
+                if (p < P) {  // uniform over the CTA
+                    float4* xrow = xrow_of(p);
+                    F4 ys[K];
+                    ypass(p, ys, xrow);
+                    __syncthreads();  // xs complete; every warp is done reading this raw stage
+                    if (issuer && p + STAGES < P) issue(p + STAGES);
+                    if (owner) xzpass(p, s, ys, xrow);
+                }
+            }
+        }
+    } else {
+        // Two planes per barrier: half the block-wide synchronisations and twice the independent
+        // arithmetic between them.
+        for (int pg = 0; pg < P; pg += LR) {
+#pragma unroll
+            for (int s2 = 0; s2 < LR / 2; ++s2) {
+                const int p0 = pg + 2 * s2;
+                if (p0 < P) {  // uniform over the CTA
+                    const bool two = p0 + 1 < P;
+                    float4* xr0 = xrow_of(p0);
+                    float4* xr1 = xrow_of(p0 + 1);
+                    F4 ys0[K], ys1[K];
+                    ypass(p0, ys0, xr0);
+                    if (two) ypass(p0 + 1, ys1, xr1);
+                    __syncthreads();
+                    if (issuer) {
+                        if (p0 + STAGES < P) issue(p0 + STAGES);
+                        if (p0 + 1 + STAGES < P) issue(p0 + 1 + STAGES);
                     }
-                    // ---- z pass: register ring, packed f32x2 ----
-                    if (p >= 2 * R) {
-                        float* orow = dst + (size_t)(rev ? z_start + nplanes - 1 - (p - 2 * R) : z_start + p - 2 * R) * plane;
-#pragma unroll
-                        for (int j = 0; j < K; ++j) {
-                            const F4& c = ring[(s - R + L) % L][j];
-                            float2 a = __fmul2_rn(w2[0], c.a), b = __fmul2_rn(w2[0], c.b);
-#pragma unroll
-                            for (int k = 1; k <= R; ++k) {
-                                const F4& lo = ring[(s - R - k + 2 * L) % L][j];
-                                const F4& hi = ring[(s - R + k + L) % L][j];
-                                a = __ffma2_rn(w2[k], __fadd2_rn(lo.a, hi.a), a);
-                                b = __ffma2_rn(w2[k], __fadd2_rn(lo.b, hi.b), b);
-                            }
-                            if (y0 + rg * K + j < d.ny)
-                                *reinterpret_cast<float4*>(orow + (size_t)j * d.nx) = make_float4(a.x, a.y, b.x, b.y);
-                        }
+                    if (owner) {
+                        xzpass(p0, 2 * s2, ys0, xr0);
+                        if (two) xzpass(p0 + 1, 2 * s2 + 1, ys1, xr1);
                     }
                 }
             }
@@ -229,9 +265,9 @@ __global__ void __launch_bounds__(32 * (RG + 1), MINB)
     }
 }
 
-template <int R, int K, int RG, int STAGES, int MINB>
+template <int R, int K, int RG, int STAGES, int MINB, int PAIR = 1>
 int launch_cfg(const SmoothArgs& a, int zc, cudaStream_t st) {
-    using C = Cfg<R, K, RG, STAGES>;
+    using C = Cfg<R, K, RG, STAGES, PAIR>;
     const Dims d = a.d;
     alignas(64) CUtensorMap map;
     const unsigned long long gdim[4] = {(unsigned long long)d.nx, (unsigned long long)d.ny, (unsigned long long)d.nz,
@@ -240,18 +276,18 @@ int launch_cfg(const SmoothArgs& a, int zc, cudaStream_t st) {
     if (!tma::encode_f32(&map, a.in, 4, gdim, box)) return 0;
     static bool attr_set = false;
     if (!attr_set) {
-        if (cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM) !=
+        if (cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES, MINB, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM) !=
             cudaSuccess) {
             cudaGetLastError();
             return 0;
         }
-        cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES, MINB>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES, MINB, PAIR>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
         attr_set = true;
         if (getenv("DEMONS_DEBUG")) {
             int nb = -1;
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_smooth_tma<R, K, RG, STAGES, MINB>, C::THREADS, C::SMEM);
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_smooth_tma<R, K, RG, STAGES, MINB, PAIR>, C::THREADS, C::SMEM);
             cudaFuncAttributes fa;
-            cudaFuncGetAttributes(&fa, k_smooth_tma<R, K, RG, STAGES, MINB>);
+            cudaFuncGetAttributes(&fa, k_smooth_tma<R, K, RG, STAGES, MINB, PAIR>);
             fprintf(stderr, "[demons] k_smooth_tma<R=%d,K=%d,RG=%d>: %d regs, %d B dyn smem, %d threads -> %d CTAs/SM\n", R, K, RG,
                     fa.numRegs, C::SMEM, C::THREADS, nb);
         }
@@ -263,7 +299,7 @@ int launch_cfg(const SmoothArgs& a, int zc, cudaStream_t st) {
     Taps t;
     for (int k = 0; k < 8; ++k) t.w[k] = k <= a.R ? a.w[k] : 0.f;
     const dim3 grid(tiles_x * tiles_y, chunks, a.ncomp);
-    k_smooth_tma<R, K, RG, STAGES, MINB><<<grid, C::THREADS, C::SMEM, st>>>(map, a.out, d, zc, tiles_x, t, a.skip, a.ascending ? 0 : 1);
+    k_smooth_tma<R, K, RG, STAGES, MINB, PAIR><<<grid, C::THREADS, C::SMEM, st>>>(map, a.out, d, zc, tiles_x, t, a.skip, a.ascending ? 0 : 1);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
@@ -303,11 +339,17 @@ int launch_smooth_tma(const SmoothArgs& a, cudaStream_t st) {
     if (a.tune == 1) {  // one large CTA per SM (tuning reference)
         if (a.R == 3) return launch_cfg<3, 2, 8, 4, 1>(a, zc, st);
     }
+    if (((a.tune >> 16) & 0xF) == 1) {  // tuning experiments: one plane per barrier
+        if (a.R == 3) return launch_cfg<3, 2, 4, 4, 3, 1>(a, zc, st);
+        if (a.R == 4) return launch_cfg<4, 2, 4, 4, 2, 1>(a, zc, st);
+    }
+    // two planes per barrier where the registers allow it: 39.6 against 41.8 us at sigma 1 (R = 3),
+    // 50.0 against 51.9 us at sigma 1.3 (R = 4), 256x256x100; no difference at R <= 2
     switch (a.R) {
-    case 1: return launch_cfg<1, 2, 4, 4, 3>(a, zc, st);
-    case 2: return launch_cfg<2, 2, 4, 4, 3>(a, zc, st);
-    case 3: return launch_cfg<3, 2, 4, 4, 3>(a, zc, st);
-    case 4: return launch_cfg<4, 2, 4, 4, 2>(a, zc, st);
+    case 1: return launch_cfg<1, 2, 4, 4, 3, 2>(a, zc, st);
+    case 2: return launch_cfg<2, 2, 4, 4, 3, 2>(a, zc, st);
+    case 3: return launch_cfg<3, 2, 4, 4, 3, 2>(a, zc, st);
+    case 4: return launch_cfg<4, 2, 4, 4, 2, 2>(a, zc, st);
     case 5: return launch_cfg<5, 2, 8, 3, 1>(a, zc, st);
     case 6: return launch_cfg<6, 2, 8, 3, 1>(a, zc, st);
     default: return 0;
