@@ -375,29 +375,47 @@ __global__ void __launch_bounds__(BX* BY) k_warp_lc(const KParams p) {
     const int zb = blockIdx.z * p.zper, ze = min(d.nz, zb + p.zper);
     const unsigned plane = (unsigned)(d.nx * d.ny);
     unsigned row = (unsigned)((zb * d.ny + y) * d.nx + xb);
-    for (int z = zb; z < ze; ++z, row += plane) {
+    constexpr int NF = IC ? 2 : 1;  // fields: u warps M, u_b warps S
+    float nux[NF][XPT], nuy[NF][XPT], nuz[NF][XPT];  // the field(s) of the next plane (register prefetch)
+    auto load_u = [&](unsigned rw) {
 #pragma unroll
-        for (int pass = 0; pass < (IC ? 2 : 1); ++pass) {
-            const float* u = pass == 0 ? p.u_in : p.ub_in;
-            const float* I = pass == 0 ? p.M : p.S;
-            float* out = (pass == 0 ? p.Mw : p.Sw) + row;
-            const float *q0 = u + row, *q1 = u + (N + row), *q2 = u + (2 * N + row);
-            float ux[XPT], uy[XPT], uz[XPT], v[XPT];
+        for (int f = 0; f < NF; ++f) {
+            const float* u = f == 0 ? p.u_in : p.ub_in;
+            const float *q0 = u + rw, *q1 = u + (N + rw), *q2 = u + (2 * N + rw);
 #pragma unroll
             for (int j = 0; j < XPT; ++j) {
                 const bool ok = FULL || r.ok[j];
-                ux[j] = ok ? __ldg(q0 + 32 * j) : 0.f;
-                uy[j] = ok ? __ldg(q1 + 32 * j) : 0.f;
-                uz[j] = ok ? __ldg(q2 + 32 * j) : 0.f;
+                nux[f][j] = ok ? __ldg(q0 + 32 * j) : 0.f;
+                nuy[f][j] = ok ? __ldg(q1 + 32 * j) : 0.f;
+                nuz[f][j] = ok ? __ldg(q2 + 32 * j) : 0.f;
             }
-            if (TEX && pass == 0) {
+        }
+    };
+    load_u(row);
+    for (int z = zb; z < ze; ++z, row += plane) {
+        float ux[NF][XPT], uy[NF][XPT], uz[NF][XPT];
+#pragma unroll
+        for (int f = 0; f < NF; ++f)
+#pragma unroll
+            for (int j = 0; j < XPT; ++j) {
+                ux[f][j] = nux[f][j];
+                uy[f][j] = nuy[f][j];
+                uz[f][j] = nuz[f][j];
+            }
+        if (z + 1 < ze) load_u(row + plane);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+            const float* I = f == 0 ? p.M : p.S;
+            float* out = (f == 0 ? p.Mw : p.Sw) + row;
+            float v[XPT];
+            if (TEX && f == 0) {
 #pragma unroll
                 for (int j = 0; j < XPT; ++j)
-                    v[j] = tex3D<float>(p.texM, xs[j] + ux[j] + 0.5f, y + uy[j] + 0.5f, z + uz[j] + 0.5f);
+                    v[j] = tex3D<float>(p.texM, xs[j] + ux[f][j] + 0.5f, y + uy[f][j] + 0.5f, z + uz[f][j] + 0.5f);
             } else {
                 unsigned o[XPT];
                 float fx[XPT], fy[XPT], fz[XPT], c[XPT][8];
-                make_cells<XPT>(d, xs, y, z, ux, uy, uz, o, fx, fy, fz);
+                make_cells<XPT>(d, xs, y, z, ux[f], uy[f], uz[f], o, fx, fy, fz);
 #pragma unroll
                 for (int j = 0; j < XPT; ++j) load_cell(I, d, o[j], c[j]);
 #pragma unroll
@@ -655,12 +673,36 @@ int launch_lc(const ForceArgs& a, const KParams& p0, bool vec4, cudaStream_t st)
     if (a.ev_mid) cudaEventRecord(a.ev_mid, st);
     p = p0;
     const dim3 block(BX, BY);
-    const dim3 agrid = force_grid(a.d, vec4 ? 4 : 1, p.zper);
+    // the stencil pass marches too: same one-wave sizing, 8-row blocks (its float4 tiles are fixed)
+    auto run_active = [&](auto kernel) {
+        const int vec = vec4 ? 4 : 1;
+        const dim3 g1 = force_grid(a.d, vec, 1);
+        int per_sm = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, BX * BY, 0) != cudaSuccess || per_sm < 1) {
+            cudaGetLastError();
+            per_sm = 1;
+        }
+        const long long slots = (long long)sm_count() * per_sm, xy = (long long)g1.x * g1.y;
+        const long long cap = force_partial_blocks(a.d);
+        int best = a.d.nz;
+        long long best_cost = -1;
+        for (int chunks = 1; chunks <= a.d.nz; ++chunks) {
+            const int zper = a.zper >= 1 ? a.zper : (a.d.nz + chunks - 1) / chunks;
+            const long long blocks = xy * ((a.d.nz + zper - 1) / zper);
+            if (blocks <= cap) {
+                const long long cost = ((blocks + slots - 1) / slots) * (zper + 2);
+                if (best_cost < 0 || cost < best_cost) best_cost = cost, best = zper;
+            }
+            if (a.zper >= 1) break;
+        }
+        p.zper = best;
+        kernel<<<force_grid(a.d, vec, best), block, 0, st>>>(p);
+    };
     switch (a.variant) {
-    case 2: if (vec4) k_force_active<2, 4><<<agrid, block, 0, st>>>(p); else k_force_active<2, 1><<<agrid, block, 0, st>>>(p); break;
-    case 3: if (vec4) k_force_active<3, 4><<<agrid, block, 0, st>>>(p); else k_force_active<3, 1><<<agrid, block, 0, st>>>(p); break;
-    case 4: if (vec4) k_force_active<4, 4><<<agrid, block, 0, st>>>(p); else k_force_active<4, 1><<<agrid, block, 0, st>>>(p); break;
-    case 5: if (vec4) k_force_active<5, 4><<<agrid, block, 0, st>>>(p); else k_force_active<5, 1><<<agrid, block, 0, st>>>(p); break;
+    case 2: if (vec4) run_active(k_force_active<2, 4>); else run_active(k_force_active<2, 1>); break;
+    case 3: if (vec4) run_active(k_force_active<3, 4>); else run_active(k_force_active<3, 1>); break;
+    case 4: if (vec4) run_active(k_force_active<4, 4>); else run_active(k_force_active<4, 1>); break;
+    case 5: if (vec4) run_active(k_force_active<5, 4>); else run_active(k_force_active<5, 1>); break;
     default: return -1;
     }
     return 2;
