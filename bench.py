@@ -44,13 +44,18 @@ def measured_peak():
 
 
 def ncu_traffic(kernel_key):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture."""
-    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
+    (profiles/r01_ncu_traffic.csv; the command that made it is in profiles/r01_ncu_full_bench.md)."""
+    path = os.path.join(ROOT, "profiles", "r01_ncu_traffic.csv")
     try:
         with open(path) as fh:
-            return json.load(fh).get(kernel_key)
+            for line in fh:
+                parts = line.strip().split(",")
+                if len(parts) == 2 and parts[0] == kernel_key:
+                    return float(parts[1])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler(threading.Thread):
