@@ -334,31 +334,46 @@ def main():
 
 
 def bench_variants(torch, B, phantoms, replicas, S, M, d_known, device, stream):
-    """BASELINE.json configs 3-4: every variant, three-level pyramid, 100 iterations per level."""
+    """BASELINE.json config 3 (variants 0-4 on the 256x256x100 pair) and config 4 (inverse consistent on
+    the 256x256x110 pair, seed 404): three-level pyramid, 100 iterations per level."""
     out = {}
     iters = [100, 100, 100]
     cases = [(0, 1.0, "passive"), (1, 1.0, "evolved_passive"), (2, 1.0, "active"), (3, 1.0, "double"),
-             (4, 0.4, "adjusted_double_a0.4"), (5, 1.0, "inverse_consistent")]
-    dS, dM = torch.from_numpy(S).to(device), torch.from_numpy(M).to(device)
-    pts = phantoms.eval_points(DIMS, np.random.default_rng(2020), 1000)
-    dpts = torch.from_numpy(pts.astype(np.float32)).to(device)
-    dtruth = torch.from_numpy(phantoms.true_inverse_at(d_known, pts).astype(np.float32)).to(device)
-    derr = torch.zeros(1000, dtype=torch.float64, device=device)
+             (4, 0.4, "adjusted_double_a0.4"), (4, 1.0, "adjusted_double_a1.0"), (5, 1.0, "inverse_consistent_256x256x110")]
+    pair = {}
     for variant, alpha, name in cases:
-        eng = B.Demons(DIMS, SPACING, variant, alpha, SIGMA, levels=3, device=device)
-        du = torch.zeros((3,) + S.shape, dtype=torch.float32, device=device)
+        dims = (256, 256, 110) if variant == 5 else DIMS
+        if dims not in pair:
+            Sx, Mx, dx = (S, M, d_known) if dims == DIMS else phantoms.lung_pair(dims, 404)
+            pts = phantoms.eval_points(dims, np.random.default_rng(2020), 1000)
+            pair = {dims: (torch.from_numpy(Sx).to(device), torch.from_numpy(Mx).to(device),
+                           torch.from_numpy(pts.astype(np.float32)).to(device),
+                           torch.from_numpy(phantoms.true_inverse_at(dx, pts).astype(np.float32)).to(device))}
+        dS, dM, dpts, dtruth = pair[dims]
+        derr = torch.zeros(1000, dtype=torch.float64, device=device)
+        eng = B.Demons(dims, SPACING, variant, alpha, SIGMA, levels=3, device=device)
+        du = torch.zeros((3, dims[2], dims[1], dims[0]), dtype=torch.float32, device=device)
         dub = torch.zeros_like(du) if variant == 5 else None
         secs, launches = time_registrations(torch, B, eng, dS, dM, du, dub, iters, 3, 2, stream, replicas)
         voxel_iters = 0
         for l in range(3):
             d = B.demons_level_dims(eng.ctx, l)
             voxel_iters += d[0] * d[1] * d[2] * 100
-        B.demons_point_error(eng.ctx, DIMS, du, 1000, dpts, dtruth, derr, stream)
+        B.demons_point_error(eng.ctx, dims, du, 1000, dpts, dtruth, derr, stream)
+        dval = torch.zeros(2, dtype=torch.float64, device=device)
+        B.demons_ssd(eng.ctx, dims, dS, dM, du, dub, dval, stream)
         torch.cuda.synchronize()
         e = derr.cpu().numpy()
         out[name] = {"ms_per_registration": 1e3 * secs / 3, "gvoxel_iter_per_s": 3 * voxel_iters / secs / 1e9,
-                     "launches_per_registration": launches // 3,
+                     "launches_per_registration": launches // 3, "final_ssd": float(dval[0]),
                      "err_mm_mean": float(e.mean()), "err_mm_sd": float(e.std())}
+        if variant == 5:
+            # config 4 report: |u_f(x) + u_b(x + u_f(x))|; u_f alone is half of the symmetric motion
+            # (no composite field is formed, reading A14), so its point error against the full truth is large
+            B.demons_ic_error(eng.ctx, dims, du, dub, dval, stream)
+            torch.cuda.synchronize()
+            out[name]["ic_error_voxel_mean"] = float(dval[0])
+            out[name]["ic_error_voxel_max"] = float(dval[1])
         eng.close()
     return out
 
