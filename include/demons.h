@@ -98,7 +98,12 @@ int demons_get_profile(const demons_ctx* ctx, double h_ms[4], long long h_launch
  * option only -- fails parity by design).  "generic_smooth" (default 0): always use
  * the three separable smoothing passes instead of the fused kernel.  "profile" (default 0): time
  * every kernel class with events inside demons_register (disables graphs, adds a final
- * synchronise; see demons_get_profile).  Kernel-selection knobs used by the tuning experiments and the
+ * synchronise; see demons_get_profile).  "l2_persist" (default 1): the kernels that gather from the
+ * moving image launch with an access-policy window that asks L2 to keep that image resident
+ * (persisting) while the field streams through; for this the library RAISES the device-wide limit
+ * cudaLimitPersistingL2CacheSize to the size of the moving image (capped by the device maximum, never
+ * lowered) on the first call that needs it, and demons_destroy resets the persisting lines
+ * (cudaCtxResetPersistingL2Cache).  Set it to 0 to leave the device limit alone.  Kernel-selection knobs used by the tuning experiments and the
  * tests of the fallback paths, not part of the stable interface: "no_tma", "smooth_zc",
  * "force_zper", "force_scalar", "tune".  Unknown name -> DEMONS_E_ARG. */
 int demons_set_option(demons_ctx* ctx, const char* name, int value);

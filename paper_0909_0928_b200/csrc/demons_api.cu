@@ -91,6 +91,8 @@ struct demons_ctx {
     int opt_smooth_zc = 0;
     int opt_no_tma = 0;
     int opt_tune = 0;
+    int opt_l2_persist = 1;
+    size_t l2_granted = 0;
     int opt_force_zper = 0;
     int opt_force_scalar = 0;
     std::vector<cudaEvent_t> prof_all;                               // events of the profiled call
@@ -187,6 +189,38 @@ int check_call_dims(const demons_ctx* c, const int dims[3], Dims* out) {
                     c->dims.nx, c->dims.ny, c->dims.nz);
     *out = d;
     return DEMONS_OK;
+}
+
+// L2 residency for the gathered image (option "l2_persist", default on): raise the device's persisting-L2
+// set-aside (cudaLimitPersistingL2CacheSize, never lowered here) to the size of the moving image, capped by
+// the device maximum.  Returns the bytes the gathering kernels may ask to keep resident (0 = off).
+size_t persisting_l2_bytes(const demons_ctx* c, const Dims& d) {
+    if (!c->opt_l2_persist) return 0;
+    static int max_persist = -1;
+    if (max_persist < 0) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev) != cudaSuccess) {
+            cudaGetLastError();
+            max_persist = 0;
+        }
+    }
+    if (max_persist <= 0) return 0;
+    size_t want = (nvox(d) * sizeof(float) + ((size_t)1 << 20) - 1) & ~(((size_t)1 << 20) - 1);
+    if (want > (size_t)max_persist) want = (size_t)max_persist;
+    size_t cur = 0;
+    if (cudaDeviceGetLimit(&cur, cudaLimitPersistingL2CacheSize) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    if (cur < want) {
+        if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) != cudaSuccess) {
+            cudaGetLastError();
+            return cur;
+        }
+        cur = want;
+    }
+    return cur < want ? cur : want;
 }
 
 MetricSink make_sink(const demons_ctx* c, const Partition& p, double* out, bool driver, double eps) {
@@ -307,6 +341,7 @@ int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb,
     fa.texM = c->opt_texture ? c->tex : 0;
     fa.zper = c->opt_force_zper;
     fa.tune = c->opt_tune;
+    fa.l2_persist_bytes = c->l2_granted;  // set once per registration, outside any stream capture
     fa.force_scalar = c->opt_force_scalar;
     cudaEvent_t e0 = prof_event(c, st, true);
     fa.ev_mid = c->variant >= DEMONS_ACTIVE ? prof_event(c, st, false) : nullptr;
@@ -405,6 +440,7 @@ int register_impl(demons_ctx* c, const float* dS, const float* dM, float* du, fl
                   const int* iters, double eps, double* h_stats, int* h_done, cudaStream_t st) {
     const bool ic = is_ic(c);
     const Partition p = make_partition(c, levels);
+    c->l2_granted = persisting_l2_bytes(c, c->dims);
     Control* ctl = reinterpret_cast<Control*>(c->ws + p.control);
     long long total_iters = 0;
     for (int l = 0; l < levels; ++l) total_iters += iters[l];
@@ -514,6 +550,7 @@ int demons_create(demons_ctx** out, const int dims[3], const float spacing[3], i
 
 void demons_destroy(demons_ctx* c) {
     if (!c) return;
+    if (c->l2_granted > 0) cudaCtxResetPersistingL2Cache();  // hand the persisting lines of M back to normal use
     for (auto& g : c->graphs) cudaGraphExecDestroy(g.exec);
     release_texture(c);
     prof_clear(c);
@@ -569,6 +606,7 @@ int demons_set_option(demons_ctx* c, const char* name, int value) {
     else if (!strcmp(name, "smooth_zc")) c->opt_smooth_zc = value;
     else if (!strcmp(name, "no_tma")) c->opt_no_tma = value != 0;
     else if (!strcmp(name, "tune")) c->opt_tune = value;
+    else if (!strcmp(name, "l2_persist")) c->opt_l2_persist = value != 0;
     else if (!strcmp(name, "force_zper")) c->opt_force_zper = value;
     else if (!strcmp(name, "force_scalar")) c->opt_force_scalar = value != 0;
     else return fail(DEMONS_E_ARG, "unknown option '%s'", name);
@@ -651,6 +689,7 @@ int demons_warp_force(demons_ctx* c, const int dims[3], const float* d_static, c
     fa.sink = make_sink(c, p, d_metrics, false, 0.0);
     fa.zper = c->opt_force_zper;
     fa.tune = c->opt_tune;
+    fa.l2_persist_bytes = c->l2_granted = persisting_l2_bytes(c, fa.d);
     fa.force_scalar = c->opt_force_scalar;
     if (c->opt_texture) {
         rc = bind_texture(c, d, d_moving, st);

@@ -22,6 +22,7 @@ struct ForceArgs {
     cudaEvent_t ev_mid;        // nullable: recorded between the warp and the force kernel (profiling)
     int zper;                  // > 0: planes per block (tuning); 0 = default
     int tune;                  // kernel-layout selector (tuning experiments; 0 = default)
+    size_t l2_persist_bytes;   // > 0: the gathering kernels ask L2 to keep up to this many bytes of M resident
     int force_scalar;          // 1 = take the one-voxel-per-thread kernels even when 128-bit access applies
 };
 
