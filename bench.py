@@ -150,6 +150,15 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def device_pair(torch, S, M, device):
+    """S and M in ONE device allocation, M right behind S: the library's L2 access-policy window
+    (demons.h, option "l2_persist") then keeps both images resident instead of M alone."""
+    both = torch.empty((2,) + S.shape, dtype=torch.float32, device=device)
+    both[0].copy_(torch.from_numpy(S))
+    both[1].copy_(torch.from_numpy(M))
+    return both[0], both[1]
+
+
 def time_registrations(torch, B, eng, dS, dM, du, dub, iters, steps, warmup, stream, replicas):
     """W untimed + K timed registrations; events on the launching stream; returns seconds."""
     def one():
@@ -202,7 +211,7 @@ def main():
     N = DIMS[0] * DIMS[1] * DIMS[2]
 
     S, M, _d_known = phantoms.lung_pair(DIMS, replicas.replica_seed(202, rank))
-    dS, dM = torch.from_numpy(S).to(device), torch.from_numpy(M).to(device)
+    dS, dM = device_pair(torch, S, M, device)
     du = torch.zeros((3,) + S.shape, dtype=torch.float32, device=device)
     eng = B.Demons(DIMS, SPACING, B.PASSIVE, 1.0, SIGMA, levels=1, device=device)
     stream = torch.cuda.Stream(device=device)
@@ -308,7 +317,8 @@ def main():
                                "force, single scale, 300 iterations, sigma 1.0",
                    "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "working set 210 MB (S, M, u, u') > 126 MB L2; no flush between steps",
-                   "graphs": True},
+                   "graphs": True,
+                   "layout": "S and M in one device allocation (the L2 persisting window covers both images)"},
         "clocks": clocks,
         "e2e": {"value": e2e["value"] / 1e9, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": 1e3 * e2e["seconds"] / args.steps},
@@ -346,7 +356,7 @@ def bench_variants(torch, B, phantoms, replicas, S, M, d_known, device, stream):
         if dims not in pair:
             Sx, Mx, dx = (S, M, d_known) if dims == DIMS else phantoms.lung_pair(dims, 404)
             pts = phantoms.eval_points(dims, np.random.default_rng(2020), 1000)
-            pair = {dims: (torch.from_numpy(Sx).to(device), torch.from_numpy(Mx).to(device),
+            pair = {dims: (*device_pair(torch, Sx, Mx, device),
                            torch.from_numpy(pts.astype(np.float32)).to(device),
                            torch.from_numpy(phantoms.true_inverse_at(dx, pts).astype(np.float32)).to(device))}
         dS, dM, dpts, dtruth = pair[dims]

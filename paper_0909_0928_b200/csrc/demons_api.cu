@@ -194,7 +194,7 @@ int check_call_dims(const demons_ctx* c, const int dims[3], Dims* out) {
 // L2 residency for the gathered image (option "l2_persist", default on): raise the device's persisting-L2
 // set-aside (cudaLimitPersistingL2CacheSize, never lowered here) to the size of the moving image, capped by
 // the device maximum.  Returns the bytes the gathering kernels may ask to keep resident (0 = off).
-size_t persisting_l2_bytes(const demons_ctx* c, const Dims& d) {
+size_t persisting_l2_bytes(const demons_ctx* c, const Dims& d, const float* S, const float* M) {
     if (!c->opt_l2_persist) return 0;
     static int max_persist = -1;
     if (max_persist < 0) {
@@ -206,7 +206,10 @@ size_t persisting_l2_bytes(const demons_ctx* c, const Dims& d) {
         }
     }
     if (max_persist <= 0) return 0;
-    size_t want = (nvox(d) * sizeof(float) + ((size_t)1 << 20) - 1) & ~(((size_t)1 << 20) - 1);
+    // the window covers S as well when the moving image directly follows the static one in memory
+    // (the pyramid levels and the host-staging buffers of the workspace do; see launch_lc)
+    const size_t span = images_adjacent(S, M, nvox(d)) ? (size_t)((const char*)M - (const char*)S) + nvox(d) * 4 : nvox(d) * 4;
+    size_t want = (span + ((size_t)1 << 20) - 1) & ~(((size_t)1 << 20) - 1);
     if (want > (size_t)max_persist) want = (size_t)max_persist;
     size_t cur = 0;
     if (cudaDeviceGetLimit(&cur, cudaLimitPersistingL2CacheSize) != cudaSuccess) {
@@ -440,7 +443,7 @@ int register_impl(demons_ctx* c, const float* dS, const float* dM, float* du, fl
                   const int* iters, double eps, double* h_stats, int* h_done, cudaStream_t st) {
     const bool ic = is_ic(c);
     const Partition p = make_partition(c, levels);
-    c->l2_granted = persisting_l2_bytes(c, c->dims);
+    c->l2_granted = persisting_l2_bytes(c, c->dims, dS, dM);
     Control* ctl = reinterpret_cast<Control*>(c->ws + p.control);
     long long total_iters = 0;
     for (int l = 0; l < levels; ++l) total_iters += iters[l];
@@ -689,7 +692,7 @@ int demons_warp_force(demons_ctx* c, const int dims[3], const float* d_static, c
     fa.sink = make_sink(c, p, d_metrics, false, 0.0);
     fa.zper = c->opt_force_zper;
     fa.tune = c->opt_tune;
-    fa.l2_persist_bytes = c->l2_granted = persisting_l2_bytes(c, fa.d);
+    fa.l2_persist_bytes = c->l2_granted = persisting_l2_bytes(c, fa.d, d_static, d_moving);
     fa.force_scalar = c->opt_force_scalar;
     if (c->opt_texture) {
         rc = bind_texture(c, d, d_moving, st);

@@ -26,6 +26,12 @@ struct ForceArgs {
     int force_scalar;          // 1 = take the one-voxel-per-thread kernels even when 128-bit access applies
 };
 
+// True when the moving image starts right behind the static one (at most one alignment gap): one
+// L2 access-policy window can then cover both.
+inline bool images_adjacent(const float* S, const float* M, size_t n) {
+    return S != nullptr && M > S && (size_t)((const char*)M - (const char*)S) <= n * sizeof(float) + 4096;
+}
+
 // S1-S4 (+S6).  Returns the number of kernels launched, or -1 with cudaGetLastError() set.
 int launch_warp_force(const ForceArgs& a, cudaStream_t stream);
 

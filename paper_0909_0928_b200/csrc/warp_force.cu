@@ -667,9 +667,11 @@ int launch_lc(const ForceArgs& a, const KParams& p0, bool vec4, cudaStream_t st)
         cfg.stream = st;
         cudaLaunchAttribute attr[1];
         if (a.l2_persist_bytes > 0) {
-            const size_t bytes = nvox(a.d) * sizeof(float);
+            const bool both = images_adjacent(a.S, a.M, nvox(a.d));  // S directly in front of M: keep both
+            const char* lo = reinterpret_cast<const char*>(both ? a.S : a.M);
+            const size_t bytes = (size_t)(reinterpret_cast<const char*>(a.M) - lo) + nvox(a.d) * sizeof(float);
             attr[0].id = cudaLaunchAttributeAccessPolicyWindow;
-            attr[0].val.accessPolicyWindow.base_ptr = const_cast<float*>(a.M);
+            attr[0].val.accessPolicyWindow.base_ptr = const_cast<char*>(lo);
             attr[0].val.accessPolicyWindow.num_bytes = bytes;
             attr[0].val.accessPolicyWindow.hitRatio =
                 a.l2_persist_bytes >= bytes ? 1.f : (float)((double)a.l2_persist_bytes / (double)bytes);
