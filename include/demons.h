@@ -101,9 +101,9 @@ int demons_get_profile(const demons_ctx* ctx, double h_ms[4], long long h_launch
  * synchronise; see demons_get_profile).  "l2_persist" (default 1): the kernels that gather from the
  * moving image launch with an access-policy window that asks L2 to keep that image resident
  * (persisting) while the field streams through; for this the library RAISES the device-wide limit
- * cudaLimitPersistingL2CacheSize to the size of the moving image (capped by the device maximum, never
- * lowered) on the first call that needs it, and demons_destroy resets the persisting lines
- * (cudaCtxResetPersistingL2Cache).  If d_moving starts directly behind d_static in memory (one allocation
+ * cudaLimitPersistingL2CacheSize to the size of the moving image on the first call that needs it (images
+ * larger than the device's maximum set-aside are left alone), and demons_destroy resets the persisting
+ * lines (cudaCtxResetPersistingL2Cache) and restores the limit it found.  If d_moving starts directly behind d_static in memory (one allocation
  * holding both, as the workspace's own pyramid levels and host-staging buffers do) the window covers the
  * static image as well.  Set the option to 0 to leave the device limit alone.  Kernel-selection knobs used by the tuning experiments and the
  * tests of the fallback paths, not part of the stable interface: "no_tma", "smooth_zc",

@@ -93,6 +93,8 @@ struct demons_ctx {
     int opt_tune = 0;
     int opt_l2_persist = 1;
     size_t l2_granted = 0;
+    bool l2_limit_raised = false;
+    size_t l2_prev_limit = 0;
     int opt_force_zper = 0;
     int opt_force_scalar = 0;
     std::vector<cudaEvent_t> prof_all;                               // events of the profiled call
@@ -194,7 +196,7 @@ int check_call_dims(const demons_ctx* c, const int dims[3], Dims* out) {
 // L2 residency for the gathered image (option "l2_persist", default on): raise the device's persisting-L2
 // set-aside (cudaLimitPersistingL2CacheSize, never lowered here) to the size of the moving image, capped by
 // the device maximum.  Returns the bytes the gathering kernels may ask to keep resident (0 = off).
-size_t persisting_l2_bytes(const demons_ctx* c, const Dims& d, const float* S, const float* M) {
+size_t persisting_l2_bytes(demons_ctx* c, const Dims& d, const float* S, const float* M) {
     if (!c->opt_l2_persist) return 0;
     static int max_persist = -1;
     if (max_persist < 0) {
@@ -210,7 +212,9 @@ size_t persisting_l2_bytes(const demons_ctx* c, const Dims& d, const float* S, c
     // (the pyramid levels and the host-staging buffers of the workspace do; see launch_lc)
     const size_t span = images_adjacent(S, M, nvox(d)) ? (size_t)((const char*)M - (const char*)S) + nvox(d) * 4 : nvox(d) * 4;
     size_t want = (span + ((size_t)1 << 20) - 1) & ~(((size_t)1 << 20) - 1);
-    if (want > (size_t)max_persist) want = (size_t)max_persist;
+    // Images that do not fit the set-aside whole are left alone: pinning a part of them takes L2 away from
+    // everything else (the smoothing halos, the stencils) and was 2x slower at 512x512x160.
+    if (want > (size_t)max_persist) return 0;
     size_t cur = 0;
     if (cudaDeviceGetLimit(&cur, cudaLimitPersistingL2CacheSize) != cudaSuccess) {
         cudaGetLastError();
@@ -219,11 +223,14 @@ size_t persisting_l2_bytes(const demons_ctx* c, const Dims& d, const float* S, c
     if (cur < want) {
         if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) != cudaSuccess) {
             cudaGetLastError();
-            return cur;
+            return 0;
         }
-        cur = want;
+        if (!c->l2_limit_raised) {  // remember what to restore in demons_destroy
+            c->l2_limit_raised = true;
+            c->l2_prev_limit = cur;
+        }
     }
-    return cur < want ? cur : want;
+    return want;
 }
 
 MetricSink make_sink(const demons_ctx* c, const Partition& p, double* out, bool driver, double eps) {
@@ -553,7 +560,13 @@ int demons_create(demons_ctx** out, const int dims[3], const float spacing[3], i
 
 void demons_destroy(demons_ctx* c) {
     if (!c) return;
-    if (c->l2_granted > 0) cudaCtxResetPersistingL2Cache();  // hand the persisting lines of M back to normal use
+    if (c->l2_granted > 0 || c->l2_limit_raised) {
+        // hand the persisting lines back to normal use and restore the device limit this context raised
+        // (work still running on a stream finishes correctly either way: the window is a hint)
+        cudaCtxResetPersistingL2Cache();
+        if (c->l2_limit_raised) cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, c->l2_prev_limit);
+        cudaGetLastError();
+    }
     for (auto& g : c->graphs) cudaGraphExecDestroy(g.exec);
     release_texture(c);
     prof_clear(c);

@@ -599,6 +599,20 @@ int launch_t(const ForceArgs& a, const KParams& p, cudaStream_t st) {
     }
 }
 
+size_t max_policy_window() {
+    static size_t n = 0;
+    if (n == 0) {
+        int dev = 0, v = 0;
+        cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMaxAccessPolicyWindowSize, dev) != cudaSuccess || v <= 0) {
+            cudaGetLastError();
+            v = 1 << 20;
+        }
+        n = (size_t)v;
+    }
+    return n;
+}
+
 int sm_count() {
     static int n = 0;
     if (n == 0) {
@@ -669,7 +683,12 @@ int launch_lc(const ForceArgs& a, const KParams& p0, bool vec4, cudaStream_t st)
         if (a.l2_persist_bytes > 0) {
             const bool both = images_adjacent(a.S, a.M, nvox(a.d));  // S directly in front of M: keep both
             const char* lo = reinterpret_cast<const char*>(both ? a.S : a.M);
-            const size_t bytes = (size_t)(reinterpret_cast<const char*>(a.M) - lo) + nvox(a.d) * sizeof(float);
+            size_t bytes = (size_t)(reinterpret_cast<const char*>(a.M) - lo) + nvox(a.d) * sizeof(float);
+            if (bytes > max_policy_window()) {  // large volumes: M alone, then as much of it as a window may span
+                lo = reinterpret_cast<const char*>(a.M);
+                bytes = nvox(a.d) * sizeof(float);
+                if (bytes > max_policy_window()) bytes = max_policy_window();
+            }
             attr[0].id = cudaLaunchAttributeAccessPolicyWindow;
             attr[0].val.accessPolicyWindow.base_ptr = const_cast<char*>(lo);
             attr[0].val.accessPolicyWindow.num_bytes = bytes;

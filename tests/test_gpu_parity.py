@@ -510,3 +510,28 @@ def test_unaligned_buffers_take_the_scalar_paths(torch_cuda, B, P, oracle, varia
     torch.cuda.synchronize()
     assert_close(sm.cpu().numpy(), oracle.smooth(ref_u, 1.0), "unaligned smooth", atol=2e-4)
     eng.close()
+
+
+def test_large_volume_l2_window(torch_cuda, B):
+    """512x512x160: the moving image (168 MB) is larger than an L2 access-policy window may span and than
+    the persisting set-aside; the launch must still work and the option must not change a single bit."""
+    torch = torch_cuda
+    dims = (512, 512, 160)
+    g = torch.Generator(device="cuda:0").manual_seed(7)
+    shape = (dims[2], dims[1], dims[0])
+    S = torch.randn(shape, generator=g, device="cuda:0") * 100.0
+    M = S + torch.randn(shape, generator=g, device="cuda:0") * 10.0
+    u = torch.randn((3,) + shape, generator=g, device="cuda:0") * 2.0
+    outs = []
+    for opt in (1, 0):
+        eng = B.Demons(dims, variant=0)
+        B.demons_set_option(eng.ctx, "l2_persist", opt)
+        out = torch.full_like(u, float("nan"))
+        met = torch.zeros(3, dtype=torch.float64, device="cuda:0")
+        B.demons_warp_force(eng.ctx, dims, S, M, u, out, None, None, met)
+        torch.cuda.synchronize()
+        assert bool(torch.isfinite(out).all())
+        outs.append((out, met.clone()))
+        eng.close()
+    assert torch.equal(outs[0][0], outs[1][0])
+    assert torch.equal(outs[0][1], outs[1][1])
