@@ -92,3 +92,18 @@ def test_binding_fails_loudly_without_library(B, tmp_path, monkeypatch):
     monkeypatch.setattr(B, "LIB_PATH", str(tmp_path / "missing.so"))
     with pytest.raises(ImportError):
         B.lib()
+
+
+def test_options_are_host_only_and_validated(B):
+    """demons_set_option needs no device: every documented name is accepted, anything else is an error."""
+    ctx = B.demons_create((16, 12, 8), (1.0, 1.0, 1.0), B.PASSIVE, 1.0, 1.0)
+    try:
+        for name in ("graphs", "texture", "generic_smooth", "profile", "l2_persist"):
+            B.demons_set_option(ctx, name, 0)
+            B.demons_set_option(ctx, name, 1)
+        B.demons_set_option(ctx, "texture", 0)
+        B.demons_set_option(ctx, "profile", 0)
+        with pytest.raises(B.DemonsError):
+            B.demons_set_option(ctx, "no_such_option", 1)
+    finally:
+        B.demons_destroy(ctx)
