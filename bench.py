@@ -8,7 +8,12 @@ iteration runs the fused warp+gradient+force+update kernel (with the SSD / relat
 reduction) and the Gaussian smoothing of the field.  `value` is Gvoxel-iterations/s with the
 inputs resident in HBM; `e2e` is the same through demons_register_host with pinned HOST buffers.
 The multi-level variants of configs 3-4 (restrict / prolong included) are timed after the main
-region and reported under "variants".  N > 1: N independent replicas, one process per GPU.
+region and reported under "variants" (with the 3D error at 1,000 seeded points against the known
+field, the final SSD and, for config 4, the inverse-consistency error); "evaluation" holds the
+same protocol for the timed config-2 registration.  "roofline" is per kernel class: algorithmic
+bytes / (share of the event-bracketed pass x iteration time of the timed region).  S and M live in
+one device allocation so that the library's L2 access-policy window keeps both resident.
+N > 1: N independent replicas, one process per GPU.
 """
 from __future__ import annotations
 
