@@ -395,6 +395,11 @@ bool capturable(cudaStream_t st) { return st != nullptr && st != cudaStreamLegac
 
 int run_level(demons_ctx* c, const Partition& p, const LevelBuffers& lb, int iters, double eps, cudaStream_t st) {
     int done = 0;
+    if (c->variant == DEMONS_EVOLVED_PASSIVE && iters > 0) {  // |grad M0|^2 of this level, fixed for the level
+        if (launch_grad_mag2(lb.d, lb.M, reinterpret_cast<float*>(c->ws + p.Mw), st) < 0)
+            return fail(DEMONS_E_CUDA, "gradient launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        c->launches += 1;
+    }
     const int chunk = iters >= 20 ? 20 : iters;
     if (c->opt_graphs && capturable(st) && iters >= 4 && !c->opt_texture && !c->opt_profile) {
         GraphEntry* ge = nullptr;
@@ -711,6 +716,11 @@ int demons_warp_force(demons_ctx* c, const int dims[3], const float* d_static, c
         rc = bind_texture(c, d, d_moving, st);
         if (rc != DEMONS_OK) return rc;
         fa.texM = c->tex;
+    }
+    if (c->variant == DEMONS_EVOLVED_PASSIVE) {
+        if (launch_grad_mag2(d, d_moving, fa.Mw, st) < 0)
+            return fail(DEMONS_E_CUDA, "gradient launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        c->launches += 1;
     }
     const int n = launch_warp_force(fa, st);
     if (n < 0) return fail(DEMONS_E_CUDA, "warp_force launch failed: %s", cudaGetErrorString(cudaGetLastError()));

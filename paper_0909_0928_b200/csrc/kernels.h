@@ -35,6 +35,10 @@ inline bool images_adjacent(const float* S, const float* M, size_t n) {
 // S1-S4 (+S6).  Returns the number of kernels launched, or -1 with cudaGetLastError() set.
 int launch_warp_force(const ForceArgs& a, cudaStream_t stream);
 
+// Variant 1, once per level (and per standalone demons_warp_force call): a.Mw <- |grad M|^2, which
+// launch_warp_force then reads instead of stencilling M (Eq.(2) uses only the magnitude of grad M0).
+int launch_grad_mag2(const Dims& d, const float* I, float* out, cudaStream_t stream);
+
 // Number of per-block partial slots launch_warp_force may use for dims d.
 int force_partial_blocks(const Dims& d);
 

@@ -70,6 +70,7 @@ struct KParams {
     float* ub_out;
     float* Mw;
     float* Sw;
+    const float* gm2;  // variant 1 (fast path): |grad M|^2 of the level, [N]
     MetricSink sink;
     cudaTextureObject_t texM;
     int zper;  // consecutive planes per block
@@ -222,7 +223,7 @@ template <int VARIANT, int XPT>
 struct PlaneRegs {
     float ux[XPT], uy[XPT], uz[XPT];
     Stencil<XPT> ss;
-    Stencil<VARIANT == 1 ? XPT : 1> ms;  // variant 1: stencil of the unwarped M (reading A4)
+    float m2[VARIANT == 1 ? XPT : 1];  // variant 1: |grad M0|^2 at the grid point (precomputed per level)
     float c[XPT][8], fx[XPT], fy[XPT], fz[XPT];
 };
 
@@ -250,7 +251,7 @@ __global__ void __launch_bounds__(BX* BY, MINB) k_force_fixed_lc(const KParams p
         const unsigned row0 = (unsigned)((zb * d.ny + y) * d.nx + xb);
         const unsigned dym = y > 0 ? (unsigned)d.nx : 0u, dyp = y < d.ny - 1 ? (unsigned)d.nx : 0u;
         float nux[XPT], nuy[XPT], nuz[XPT];  // field of the plane after the one being issued
-        float sm[XPT], sc[XPT], mm[XPT], mc[XPT];  // centre values of planes z-1 and z (S; M for variant 1)
+        float sm[XPT], sc[XPT];  // centre values of S on planes z-1 and z
 
         const bool rt = p.zper > 0;  // always true; opaque to the compiler (see above)
         auto load_u = [&](unsigned row) {
@@ -276,7 +277,11 @@ __global__ void __launch_bounds__(BX* BY, MINB) k_force_fixed_lc(const KParams p
             if (z + 1 < ze) load_u(row + plane);
             if (rt) {
                 load_stencil<XPT, FULL>(p.S, r, row, dym, dyp, dzp, q.ss);
-                if constexpr (VARIANT == 1) load_stencil<XPT, FULL>(p.M, r, row, dym, dyp, dzp, q.ms);
+                if constexpr (VARIANT == 1) {
+                    const float* pg = p.gm2 + row;
+#pragma unroll
+                    for (int j = 0; j < XPT; ++j) q.m2[j] = (FULL || r.ok[j]) ? __ldg(pg + 32 * j) : 0.f;
+                }
             }
             if constexpr (!TEX) {
                 unsigned o[XPT];
@@ -308,12 +313,9 @@ __global__ void __launch_bounds__(BX* BY, MINB) k_force_fixed_lc(const KParams p
                 if constexpr (VARIANT == 0) {
                     k = guarded_div(dd, fmaf(dd, dd, g2));  // Eq.(1)
                 } else {
-                    // Eq.(2), gM0 = gradient of the UNWARPED level moving image (reading A4)
-                    const float hx = 0.5f * (q.ms.xr[j] - q.ms.xl[j]), hy = 0.5f * (q.ms.yp[j] - q.ms.ym[j]),
-                                hz = 0.5f * (q.ms.zp[j] - mm[j]);
-                    mm[j] = mc[j];
-                    mc[j] = q.ms.zp[j];
-                    const float m2 = fmaf(hx, hx, fmaf(hy, hy, hz * hz));
+                    // Eq.(2) needs only |gM0|, the gradient magnitude of the UNWARPED level moving image at the grid
+                    // point (reading A4): fixed for the level, so it is read from a precomputed volume
+                    const float m2 = q.m2[j];
                     const float num = 4.f * dd * fast_sqrt(g2) * fast_sqrt(m2);
                     const float den = (fmaf(2.f * dd, dd, g2 + m2)) * (g2 + m2);
                     k = guarded_div(num, den);
@@ -335,16 +337,11 @@ __global__ void __launch_bounds__(BX* BY, MINB) k_force_fixed_lc(const KParams p
         load_u(row0);
         {
             const float *qs = p.S + row0, *qsm = p.S + (row0 - (zb > 0 ? plane : 0u));
-            const float *qm = p.M + row0, *qmm = p.M + (row0 - (zb > 0 ? plane : 0u));
 #pragma unroll
             for (int j = 0; j < XPT; ++j) {
                 const bool ok = FULL || r.ok[j];
                 sc[j] = ok ? __ldg(qs + 32 * j) : 0.f;
                 sm[j] = ok ? __ldg(qsm + 32 * j) : 0.f;
-                if constexpr (VARIANT == 1) {
-                    mc[j] = ok ? __ldg(qm + 32 * j) : 0.f;
-                    mm[j] = ok ? __ldg(qmm + 32 * j) : 0.f;
-                }
             }
         }
         PlaneRegs<VARIANT, XPT> q;
@@ -357,6 +354,17 @@ __global__ void __launch_bounds__(BX* BY, MINB) k_force_fixed_lc(const KParams p
         if (block_reduce_publish<3>(acc, p.sink.partials, p.sink.stride, p.sink.ticket))
             publish_metrics(acc, p.sink);
     }
+}
+
+// |grad M|^2 of a level image (central differences, clamped; O1), once per level for variant 1.
+__global__ void __launch_bounds__(256) k_grad_mag2(const float* __restrict__ I, float* __restrict__ out, const Dims d) {
+    const int x = blockIdx.x * 64 + threadIdx.x, y = blockIdx.y * 4 + threadIdx.y, z = blockIdx.z;
+    if (x >= d.nx || y >= d.ny) return;
+    const unsigned plane = (unsigned)(d.nx * d.ny), i = (unsigned)((z * d.ny + y) * d.nx + x);
+    const float gx = 0.5f * (__ldg(I + i + (x < d.nx - 1)) - __ldg(I + i - (x > 0)));
+    const float gy = 0.5f * (__ldg(I + i + (y < d.ny - 1 ? d.nx : 0)) - __ldg(I + i - (y > 0 ? d.nx : 0)));
+    const float gz = 0.5f * (__ldg(I + i + (z < d.nz - 1 ? plane : 0u)) - __ldg(I + i - (z > 0 ? plane : 0u)));
+    out[i] = fmaf(gx, gx, fmaf(gy, gy, gz * gz));
 }
 
 // Pass 1 of variants 2-5 in the same layout: Mw = warp(M, u)  (variant 5 also Sw = warp(S, ub)).
@@ -754,18 +762,14 @@ int launch_lc(const ForceArgs& a, const KParams& p0, bool vec4, cudaStream_t st)
 template <bool TEX>
 int launch_lc_x(const ForceArgs& a, const KParams& p, bool vec4, cudaStream_t st) {
     int xpt = a.d.nx <= 32 ? 1 : a.d.nx <= 64 ? 2 : 4;
-    // Evolved passive (two stencils): 2 voxels per lane at 128 registers -- 4 voxels spill (84 us), 2 voxels
-    // at 80 registers spill too (80 us), 2 voxels at 128 registers do not (65 us, 256x256x100).
-    const bool two = a.variant == 1;
-    if (two && xpt > 2) xpt = 2;
     if ((a.tune >> 4) & 0xF) xpt = (a.tune >> 4) & 0xF;  // tuning experiments
     if (a.d.nx % (32 * xpt) == 0) {
         if (xpt == 1) return launch_lc<1, true, TEX, 3>(a, p, vec4, st);
-        if (xpt == 2) return two ? launch_lc<2, true, TEX, 2>(a, p, vec4, st) : launch_lc<2, true, TEX, 3>(a, p, vec4, st);
+        if (xpt == 2) return launch_lc<2, true, TEX, 3>(a, p, vec4, st);
         return launch_lc<4, true, TEX, 2>(a, p, vec4, st);
     }
     if (xpt == 1) return launch_lc<1, false, TEX, 3>(a, p, vec4, st);
-    if (xpt == 2) return two ? launch_lc<2, false, TEX, 2>(a, p, vec4, st) : launch_lc<2, false, TEX, 3>(a, p, vec4, st);
+    if (xpt == 2) return launch_lc<2, false, TEX, 3>(a, p, vec4, st);
     return launch_lc<4, false, TEX, 2>(a, p, vec4, st);
 }
 
@@ -781,6 +785,12 @@ int force_partial_blocks(const Dims& d) {
     return (int)(n > scalar ? n : scalar);
 }
 
+int launch_grad_mag2(const Dims& d, const float* I, float* out, cudaStream_t st) {
+    const dim3 grid((d.nx + 63) / 64, (d.ny + 3) / 4, d.nz);
+    k_grad_mag2<<<grid, dim3(64, 4), 0, st>>>(I, out, d);
+    return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+}
+
 int launch_warp_force(const ForceArgs& a, cudaStream_t st) {
     KParams p;
     p.d = a.d;
@@ -793,6 +803,7 @@ int launch_warp_force(const ForceArgs& a, cudaStream_t st) {
     p.ub_out = a.ub_out;
     p.Mw = a.Mw;
     p.Sw = a.Sw;
+    p.gm2 = a.Mw;  // variants 0-1 do not materialise Mw: the buffer holds |grad M|^2 (launch_grad_mag2)
     p.sink = a.sink;
     p.texM = a.texM;
     // planes per block: at least ZPER (never more blocks than force_partial_blocks() promised),

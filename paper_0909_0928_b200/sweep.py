@@ -22,7 +22,9 @@ import numpy as np
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 SEEDS = {(128, 128, 64): 500, (256, 256, 100): 501, (512, 512, 160): 502, (512, 512, 256): 503}
 # algorithmic bytes per voxel of each entry point as implemented
-FORCE_BYTES = {0: 32.0, 1: 32.0, 2: 52.0, 3: 52.0, 4: 52.0, 5: 96.0}
+# variant 1 through the standalone entry point: |grad M|^2 pass (4 in, 4 out) + fused pass (u 12, S 4, M 4,
+# |grad M|^2 4 in, 12 out); inside a registration the first pass runs once per level, not per iteration
+FORCE_BYTES = {0: 32.0, 1: 44.0, 2: 52.0, 3: 52.0, 4: 52.0, 5: 96.0}
 VARIANT_NAMES = ["passive", "evolved_passive", "active", "double", "adjusted_double", "inverse_consistent"]
 
 
