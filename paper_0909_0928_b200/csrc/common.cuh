@@ -146,11 +146,17 @@ __device__ __forceinline__ void load_cell(const float* __restrict__ I, const Dim
     c[4] = __ldg(r01), c[5] = __ldg(r01 + 1), c[6] = __ldg(r11), c[7] = __ldg(r11 + 1);
 }
 
-// Interpolation along x, then y, then z (O2).
+// Interpolation along x, then y, then z (O2).  The two z planes go through the x and y lerps as packed
+// f32x2 pairs (FFMA2 on sm_100): 8 instructions instead of 14, the same roundings as 7 scalar lerp1.
+__device__ __forceinline__ float2 lerp1x2(float2 a, float2 b, float t) {
+    const float2 t2 = make_float2(t, t), nt2 = make_float2(-t, -t);
+    return __ffma2_rn(t2, b, __ffma2_rn(nt2, a, a));
+}
 __device__ __forceinline__ float lerp_cell(const float (&c)[8], float fx, float fy, float fz) {
-    const float a00 = lerp1(c[0], c[1], fx), a10 = lerp1(c[2], c[3], fx);
-    const float a01 = lerp1(c[4], c[5], fx), a11 = lerp1(c[6], c[7], fx);
-    return lerp1(lerp1(a00, a10, fy), lerp1(a01, a11, fy), fz);
+    const float2 x0 = lerp1x2(make_float2(c[0], c[4]), make_float2(c[1], c[5]), fx);  // (a00, a01)
+    const float2 x1 = lerp1x2(make_float2(c[2], c[6]), make_float2(c[3], c[7]), fx);  // (a10, a11)
+    const float2 yb = lerp1x2(x0, x1, fy);                                            // (b0, b1)
+    return lerp1(yb.x, yb.y, fz);
 }
 
 // VEC consecutive floats along x: one 128-bit access when VEC == 4.
