@@ -98,7 +98,9 @@ int demons_get_profile(const demons_ctx* ctx, double h_ms[4], long long h_launch
  * option only -- fails parity by design).  "generic_smooth" (default 0): always use
  * the three separable smoothing passes instead of the fused kernel.  "profile" (default 0): time
  * every kernel class with events inside demons_register (disables graphs, adds a final
- * synchronise; see demons_get_profile).  "l2_persist" (default 1): the kernels that gather from the
+ * synchronise; see demons_get_profile).  "zero_start" (default 0): a single-level registration starts
+ * from a zero field set on the device; d_u / h_u (and u_back) are then outputs only and
+ * demons_register_host does not upload them.  "l2_persist" (default 1): the kernels that gather from the
  * moving image launch with an access-policy window that asks L2 to keep that image resident
  * (persisting) while the field streams through; for this the library RAISES the device-wide limit
  * cudaLimitPersistingL2CacheSize to the size of the moving image on the first call that needs it (images

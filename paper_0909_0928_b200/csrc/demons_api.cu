@@ -92,6 +92,7 @@ struct demons_ctx {
     int opt_no_tma = 0;
     int opt_tune = 0;
     int opt_l2_persist = 1;
+    int opt_zero_start = 0;
     size_t l2_granted = 0;
     bool l2_limit_raised = false;
     size_t l2_prev_limit = 0;
@@ -480,7 +481,7 @@ int register_impl(demons_ctx* c, const float* dS, const float* dM, float* du, fl
         c->launches += 2;
         prof_pair(c, PROF_PYRAMID, e0, prof_event(c, st, true));
     }
-    if (levels > 1) {  // the coarsest level starts from zero (O9)
+    if (levels > 1 || c->opt_zero_start) {  // the coarsest level starts from zero (O9); "zero_start": a single level too
         const size_t n = nvox(lb[levels - 1].d);
         CUDA_TRY(cudaMemsetAsync(lb[levels - 1].u, 0, 3 * n * 4, st));
         if (ic) CUDA_TRY(cudaMemsetAsync(lb[levels - 1].ub, 0, 3 * n * 4, st));
@@ -628,6 +629,7 @@ int demons_set_option(demons_ctx* c, const char* name, int value) {
     else if (!strcmp(name, "no_tma")) c->opt_no_tma = value != 0;
     else if (!strcmp(name, "tune")) c->opt_tune = value;
     else if (!strcmp(name, "l2_persist")) c->opt_l2_persist = value != 0;
+    else if (!strcmp(name, "zero_start")) c->opt_zero_start = value != 0;
     else if (!strcmp(name, "force_zper")) c->opt_force_zper = value;
     else if (!strcmp(name, "force_scalar")) c->opt_force_scalar = value != 0;
     else return fail(DEMONS_E_ARG, "unknown option '%s'", name);
@@ -659,7 +661,7 @@ int demons_register_host(demons_ctx* c, const float* h_static, const float* h_mo
     float* dUb = ic ? reinterpret_cast<float*>(c->ws + p.hUb) : nullptr;
     CUDA_TRY(cudaMemcpyAsync(dS, h_static, N * 4, cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemcpyAsync(dM, h_moving, N * 4, cudaMemcpyHostToDevice, st));
-    if (levels == 1) {
+    if (levels == 1 && !c->opt_zero_start) {
         CUDA_TRY(cudaMemcpyAsync(dU, h_u, 3 * N * 4, cudaMemcpyHostToDevice, st));
         if (ic) CUDA_TRY(cudaMemcpyAsync(dUb, h_u_back, 3 * N * 4, cudaMemcpyHostToDevice, st));
     }

@@ -535,3 +535,21 @@ def test_large_volume_l2_window(torch_cuda, B):
         eng.close()
     assert torch.equal(outs[0][0], outs[1][0])
     assert torch.equal(outs[0][1], outs[1][1])
+
+
+def test_zero_start_option(torch_cuda, B, P, oracle):
+    """"zero_start": the single-level registration ignores what is in u on entry (device and host paths)."""
+    torch = torch_cuda
+    S, M, _ = P.config1_pair()
+    dims = (S.shape[2], S.shape[1], S.shape[0])
+    ref = oracle.register(0, 1.0, 1.0, S, M, [8])
+    eng = B.Demons(dims, variant=0, levels=1)
+    B.demons_set_option(eng.ctx, "zero_start", 1)
+    du = torch.full((3,) + S.shape, 7.5, dtype=torch.float32, device="cuda:0")   # garbage on entry
+    B.demons_register(eng.ctx, dev(torch, S), dev(torch, M), du, None, [8])
+    torch.cuda.synchronize()
+    assert np.abs(du.cpu().numpy() - ref["u"]).max() <= 1e-3
+    hu = np.full((3,) + S.shape, -3.0, np.float32)
+    B.demons_register_host(eng.ctx, S, M, hu, None, [8])
+    assert np.array_equal(hu, du.cpu().numpy())
+    eng.close()
