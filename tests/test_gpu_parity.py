@@ -553,3 +553,29 @@ def test_zero_start_option(torch_cuda, B, P, oracle):
     B.demons_register_host(eng.ctx, S, M, hu, None, [8])
     assert np.array_equal(hu, du.cpu().numpy())
     eng.close()
+
+
+def test_texture_option_is_measured_not_parity(torch_cuda, B, P, oracle):
+    """S9: the texture-unit path (9-bit filter weights) runs, stays within a fraction of a voxel of the
+    software path, is NOT within the parity bar (that is why it is only an option), and switching it off
+    restores the software result bit for bit."""
+    torch = torch_cuda
+    dims = (64, 64, 32)
+    S, M, u, _ = make_case(P, dims, seed=3)
+    eng = B.Demons(dims, variant=0)
+    dS, dM, du = dev(torch, S), dev(torch, M), dev(torch, u)
+    met = torch.zeros(3, dtype=torch.float64, device="cuda:0")
+    soft = torch.empty_like(du)
+    B.demons_warp_force(eng.ctx, dims, dS, dM, du, soft, None, None, met)
+    B.demons_set_option(eng.ctx, "texture", 1)
+    tex = torch.empty_like(du)
+    B.demons_warp_force(eng.ctx, dims, dS, dM, du, tex, None, None, met)
+    B.demons_set_option(eng.ctx, "texture", 0)
+    again = torch.empty_like(du)
+    B.demons_warp_force(eng.ctx, dims, dS, dM, du, again, None, None, met)
+    torch.cuda.synchronize()
+    err = float((tex - soft).abs().max())
+    assert bool(torch.isfinite(tex).all()) and err < 0.5
+    assert err > 1e-4          # outside the parity bar: hardware weights have 8 fractional bits
+    assert torch.equal(again, soft)
+    eng.close()
