@@ -375,6 +375,83 @@ def test_ic_error_closed_form(oracle):
     assert abs(mean - expect) < 1e-12 and abs(mx - expect) < 1e-12
 
 
+def test_ic_error_sample_position_closed_form(oracle):
+    """BASELINE.json config 4 / PAPER.md L109: e(x) = |u_f(x) + u_b(x + u_f(x))| -- the backward field is
+    sampled at the DISPLACED position.  u_f = (a, 0, 0) constant, u_b = -(b x, 0, 0) linear in x: trilinear
+    interpolation reproduces a linear field, so e(x) = |a - b (x + a)| where x + a is inside the volume and
+    |a - b clamp(x + a)| where it is not.  A version that samples u_b at x gives |a - b x| and fails."""
+    nz, ny, nx = 5, 6, 16
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    for a, b in ((3.0, 0.25), (1.5, 0.125), (-2.25, 0.5)):   # b x is exact in fp32 for these
+        uf = np.zeros((3, nz, ny, nx), np.float32)
+        ub = np.zeros_like(uf)
+        uf[0] = a
+        ub[0] = -b * x
+        want = np.abs(a - b * np.clip(x + a, 0, nx - 1))
+        wrong = np.abs(a - b * x)
+        assert np.abs(want - wrong).max() > 0.1            # the two readings differ on this input
+        mean, mx = oracle.ic_error(uf, ub)
+        assert mean == pytest.approx(want.mean(), rel=1e-12, abs=1e-13)
+        assert mx == pytest.approx(want.max(), rel=1e-12, abs=1e-13)
+    # the same along y and z, all three components live
+    uf = np.zeros((3, nz, ny, nx), np.float32)
+    ub = np.zeros_like(uf)
+    uf[0], uf[1], uf[2] = 1.0, 2.0, -1.0
+    ub[0], ub[1], ub[2] = -0.25 * y, 0.5 * z, -0.125 * x
+    px, py, pz = np.clip(x + 1.0, 0, nx - 1), np.clip(y + 2.0, 0, ny - 1), np.clip(z - 1.0, 0, nz - 1)
+    e = np.sqrt((1.0 - 0.25 * py) ** 2 + (2.0 + 0.5 * pz) ** 2 + (-1.0 - 0.125 * px) ** 2)
+    mean, mx = oracle.ic_error(uf, ub)
+    assert mean == pytest.approx(e.mean(), rel=1e-12) and mx == pytest.approx(e.max(), rel=1e-12)
+
+
+def test_ic_error_matches_library_resampler(oracle):
+    """Random smooth fields: u_b resampled at x + u_f(x) by scipy.ndimage.map_coordinates."""
+    dims = (14, 12, 10)
+    rng = np.random.default_rng(8)
+    uf = P.bump_field(dims, rng, 5, (2.0, 5.0), 2.5, centre_frac=1.0)
+    ub = P.bump_field(dims, rng, 5, (2.0, 5.0), 2.5, centre_frac=1.0)
+    nz, ny, nx = uf.shape[1:]
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    coords = [z + uf[2].astype(np.float64), y + uf[1].astype(np.float64), x + uf[0].astype(np.float64)]
+    e2 = 0.0
+    for c in range(3):
+        s = ndimage.map_coordinates(ub[c].astype(np.float64), coords, order=1, mode="nearest")
+        e2 = e2 + (uf[c].astype(np.float64) + s) ** 2
+    e = np.sqrt(e2)
+    mean, mx = oracle.ic_error(uf, ub)
+    assert mean == pytest.approx(e.mean(), rel=1e-9) and mx == pytest.approx(e.max(), rel=1e-9)
+    # and the reading that samples at x is measurably different here
+    e_wrong = np.sqrt(((uf.astype(np.float64) + ub.astype(np.float64)) ** 2).sum(axis=0))
+    assert abs(e_wrong.mean() - mean) > 1e-3
+
+
+@pytest.mark.parametrize("variant", [0, 5])
+def test_final_ssd_matches_library_resampler(oracle, variant):
+    """O8 final SSD = sum (warp(M,u) - S)^2 (variant 5: (warp(M,u) - warp(S,ub))^2), restated with
+    scipy.ndimage.map_coordinates (order 1, clamped) in double, warped values rounded to float32 as the
+    oracle stores them."""
+    dims = (18, 15, 11)
+    rng = np.random.default_rng(21)
+    S = P.blob_volume(dims, rng, 8, 10.0)
+    M = P.blob_volume(dims, rng, 8, 10.0)
+    u = P.bump_field(dims, rng, 5, (2.0, 6.0), 2.0, centre_frac=1.0)
+    ub = P.bump_field(dims, rng, 5, (2.0, 6.0), 2.0, centre_frac=1.0)
+    nz, ny, nx = S.shape
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+
+    def lib_warp(I, f):
+        coords = [z + f[2].astype(np.float64), y + f[1].astype(np.float64), x + f[0].astype(np.float64)]
+        return ndimage.map_coordinates(I.astype(np.float64), coords, order=1, mode="nearest").astype(np.float32)
+
+    a = lib_warp(M, u).astype(np.float64)
+    b = lib_warp(S, ub).astype(np.float64) if variant == 5 else S.astype(np.float64)
+    want = ((a - b) ** 2).sum()
+    got = oracle.final_ssd(variant, S, M, u, ub if variant == 5 else None)
+    assert got == pytest.approx(want, rel=1e-6)
+    # a dropped displacement or a swapped operand is far outside that
+    assert abs(((M.astype(np.float64) - b) ** 2).sum() - want) > 1e-3 * want
+
+
 @pytest.mark.parametrize("variant", [0, 3, 5])
 def test_axis_permutation_and_mirror_equivariance(oracle, variant):  # P12
     n = 14
