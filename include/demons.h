@@ -21,8 +21,9 @@
  *  - Every function returns a DEMONS_* status; nothing throws, aborts or exits.  On failure
  *    demons_last_error() returns a thread-local description.  There is no CPU fallback: with no
  *    usable CUDA device every compute entry point returns DEMONS_E_CUDA.
- *  - Pointers that are 16-byte aligned with nx % 4 == 0 take the 128-bit vectorised kernels;
- *    anything else takes scalar kernels with identical results.
+ *  - Buffers that are 16-byte aligned with nx % 4 == 0 take the fast kernels (TMA-fed smoothing, 128-bit
+ *    rows in the stencil pass; the gathering passes use lane-consecutive 32-bit accesses, one 128-byte
+ *    line per warp); anything else takes scalar kernels with identical results.
  */
 #ifndef DEMONS_H
 #define DEMONS_H
@@ -57,8 +58,10 @@ enum {
 #define DEMONS_MAX_RADIUS 32
 /* Largest number of pyramid levels. */
 #define DEMONS_MAX_LEVELS 8
-/* Capacity of the per-iteration statistics buffer inside the workspace (rows of 3 doubles). */
+/* Capacity of the per-iteration statistics buffer inside the workspace (rows of 3 doubles, per pair). */
 #define DEMONS_MAX_STATS_ROWS 16384
+/* Largest batch of demons_register_batch. */
+#define DEMONS_MAX_BATCH 64
 
 /* ---- context ---------------------------------------------------------------------------
  * demons_create: host-only, no CUDA call.  dims = finest-level volume size (each >= 1),
@@ -75,6 +78,9 @@ void demons_destroy(demons_ctx* ctx);
  * dims and a pyramid of `levels` (1..DEMONS_MAX_LEVELS).  Includes the device staging buffers
  * of demons_register_host.  Returns 0 on bad arguments. */
 size_t demons_workspace_bytes(const demons_ctx* ctx, int levels);
+/* The same for demons_register_batch with up to `nbatch` pairs (1..DEMONS_MAX_BATCH); a workspace of this
+ * size also serves every single-registration entry point. */
+size_t demons_workspace_bytes_batch(const demons_ctx* ctx, int levels, int nbatch);
 /* d_ws: device pointer, 256-byte aligned, `bytes` >= demons_workspace_bytes(ctx, levels) for
  * the `levels` later passed to demons_register.  The library zeroes its counters on `stream`
  * lazily at first use.  The caller keeps ownership. */
@@ -105,11 +111,14 @@ int demons_get_profile(const demons_ctx* ctx, double h_ms[4], long long h_launch
  * (persisting) while the field streams through; for this the library RAISES the device-wide limit
  * cudaLimitPersistingL2CacheSize to the size of the moving image on the first call that needs it (images
  * larger than the device's maximum set-aside are left alone), and demons_destroy resets the persisting
- * lines (cudaCtxResetPersistingL2Cache) and restores the limit it found.  If d_moving starts directly behind d_static in memory (one allocation
- * holding both, as the workspace's own pyramid levels and host-staging buffers do) the window covers the
- * static image as well.  Set the option to 0 to leave the device limit alone.  Kernel-selection knobs used by the tuning experiments and the
- * tests of the fallback paths, not part of the stable interface: "no_tma", "smooth_zc",
- * "force_zper", "force_scalar", "tune".  Unknown name -> DEMONS_E_ARG. */
+ * lines (cudaCtxResetPersistingL2Cache) and restores the limit it found.  If d_moving starts directly behind
+ * d_static in memory (one allocation holding both, as the workspace's own pyramid levels and host-staging
+ * buffers do) the window covers the static image as well.  Set the option to 0 to leave the device limit
+ * alone.  "ic_one_field" (default 1): variant 5 started from zero fields (every multi-level call, and single
+ * levels under "zero_start") iterates on the forward field alone and writes u_back = -u once on exit; the two
+ * fields are exact negatives of each other at every iteration (negation commutes with every operation of the
+ * iteration), so the result is bit-identical to iterating on both (0 = always iterate on both).
+ * Unknown name -> DEMONS_E_ARG. */
 int demons_set_option(demons_ctx* ctx, const char* name, int value);
 
 /* ---- full registration (PAPER.md L123-125 multi-scale, L145 stopping rule; O9/O10) ---------
@@ -129,7 +138,20 @@ int demons_register(demons_ctx* ctx, const float* d_static, const float* d_movin
                     float* d_u_back, int levels, const int* h_iters_per_level, double eps,
                     double* h_stats, int* h_iters_done, void* stream);
 
-/* Same, with HOST buffers: copies h_static/h_moving (and, for levels == 1, h_u / h_u_back) to
+/* A batch of `nbatch` INDEPENDENT registrations of equally sized pairs in one call (many
+ * registrations per patient course; Table 2: five cases x six methods).  Layouts: d_static and
+ * d_moving [nbatch][N], d_u (and d_u_back) [nbatch][3][N], contiguous; h_stats (nullable)
+ * [nbatch][sum iters][3]; h_iters_done (nullable) [nbatch][levels].  Pyramid levels too small to fill the
+ * GPU run several pairs per kernel launch (the pair index rides in the grid); large levels run pair by
+ * pair, so that one pair's images stay resident in L2.  Each pair stops on its own when eps > 0.  The
+ * field of every pair is bit-identical to what demons_register gives for that pair alone; the statistics
+ * agree to rounding (the block partition of the reduction differs).  Needs a workspace of
+ * demons_workspace_bytes_batch(ctx, levels, nbatch).  The "texture" option serves nbatch == 1 only. */
+int demons_register_batch(demons_ctx* ctx, int nbatch, const float* d_static, const float* d_moving, float* d_u,
+                          float* d_u_back, int levels, const int* h_iters_per_level, double eps,
+                          double* h_stats, int* h_iters_done, void* stream);
+
+/* Same as demons_register, with HOST buffers: copies h_static/h_moving (and, for levels == 1, h_u / h_u_back) to
  * staging buffers inside the workspace, registers, copies the field(s) back, synchronises.
  * Pinned host memory makes the copies asynchronous on `stream`; pageable memory also works. */
 int demons_register_host(demons_ctx* ctx, const float* h_static, const float* h_moving, float* h_u,

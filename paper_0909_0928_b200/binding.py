@@ -27,6 +27,7 @@ SIGNATURES = {
                                      ctypes.c_float]),
     "demons_destroy": (None, [_vp]),
     "demons_workspace_bytes": (ctypes.c_size_t, [_vp, ctypes.c_int]),
+    "demons_workspace_bytes_batch": (ctypes.c_size_t, [_vp, ctypes.c_int, ctypes.c_int]),
     "demons_set_workspace": (ctypes.c_int, [_vp, _vp, ctypes.c_size_t]),
     "demons_level_dims": (ctypes.c_int, [_vp, ctypes.c_int, _c_int3]),
     "demons_launch_count": (ctypes.c_longlong, [_vp]),
@@ -34,6 +35,8 @@ SIGNATURES = {
     "demons_set_option": (ctypes.c_int, [_vp, ctypes.c_char_p, ctypes.c_int]),
     "demons_register": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, ctypes.c_int, _c_int3, ctypes.c_double, _vp, _vp,
                                        _vp]),
+    "demons_register_batch": (ctypes.c_int, [_vp, ctypes.c_int, _vp, _vp, _vp, _vp, ctypes.c_int, _c_int3, ctypes.c_double,
+                                             _vp, _vp, _vp]),
     "demons_register_host": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, ctypes.c_int, _c_int3, ctypes.c_double, _vp,
                                             _vp, _vp]),
     "demons_warp_force": (ctypes.c_int, [_vp, _c_int3, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
@@ -122,6 +125,10 @@ def demons_workspace_bytes(ctx, levels):
     return int(lib().demons_workspace_bytes(ctx, int(levels)))
 
 
+def demons_workspace_bytes_batch(ctx, levels, nbatch):
+    return int(lib().demons_workspace_bytes_batch(ctx, int(levels), int(nbatch)))
+
+
 def demons_set_workspace(ctx, d_ws, nbytes):
     _check(lib().demons_set_workspace(ctx, _ptr(d_ws), int(nbytes)))
 
@@ -154,6 +161,14 @@ def demons_register(ctx, d_static, d_moving, d_u, d_u_back, iters_per_level, eps
     it = (ctypes.c_int * levels)(*[int(i) for i in iters_per_level])
     _check(lib().demons_register(ctx, _ptr(d_static), _ptr(d_moving), _ptr(d_u), _ptr(d_u_back), levels, it,
                                  float(eps), _ptr(h_stats), _ptr(h_iters_done), _stream(stream)))
+
+
+def demons_register_batch(ctx, nbatch, d_static, d_moving, d_u, d_u_back, iters_per_level, eps=0.0, h_stats=None,
+                          h_iters_done=None, stream=None):
+    levels = len(iters_per_level)
+    it = (ctypes.c_int * levels)(*[int(i) for i in iters_per_level])
+    _check(lib().demons_register_batch(ctx, int(nbatch), _ptr(d_static), _ptr(d_moving), _ptr(d_u), _ptr(d_u_back),
+                                       levels, it, float(eps), _ptr(h_stats), _ptr(h_iters_done), _stream(stream)))
 
 
 def demons_register_host(ctx, h_static, h_moving, h_u, h_u_back, iters_per_level, eps=0.0, h_stats=None,
@@ -211,14 +226,15 @@ class Demons:
     """Owns a demons_ctx and the torch tensor backing its workspace (allocation only)."""
 
     def __init__(self, dims, spacing=(1.0, 1.0, 1.0), variant=PASSIVE, alpha=1.0, sigma=1.0, levels=1,
-                 device="cuda:0"):
+                 device="cuda:0", nbatch=1):
         import torch
         self.dims = tuple(int(d) for d in dims)
         self.variant = int(variant)
         self.levels = int(levels)
         self.sigma = float(sigma)
         self.ctx = demons_create(self.dims, spacing, variant, alpha, sigma)
-        nbytes = demons_workspace_bytes(self.ctx, levels)
+        self.nbatch = int(nbatch)
+        nbytes = demons_workspace_bytes_batch(self.ctx, levels, nbatch)
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=device)
         off = (-self.workspace.data_ptr()) % 256
         self._ws_ptr = self.workspace.data_ptr() + off

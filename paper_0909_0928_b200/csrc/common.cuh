@@ -15,25 +15,37 @@ __host__ __device__ __forceinline__ size_t nvox(const Dims& d) {
     return (size_t)d.nx * (size_t)d.ny * (size_t)d.nz;
 }
 
+constexpr int LHIST = 16;  // power of two >= 11 (lag of 10 iterations)
+
+// Per-registration control block in the workspace (one per pair of a batch): block ticket of the metric
+// reduction, statistics row cursor and the state of the device-side stopping rule.
+struct Control {
+    unsigned int ticket;       // block-completion counter, left at 0 by the last block
+    unsigned int row_counter;  // next row of the statistics buffer
+    unsigned int level_iter;   // iterations executed on the current level
+    int stop_force;            // set when the stopping rule fires; force kernels then skip
+    int stop_smooth;           // set by the first skipped force kernel; smoothing then skips
+    int pad0[11];
+    int lvalid[LHIST];         // l_n defined (sum|u| > 0)
+    double lhist[LHIST];       // ring of relative norms l_n of this level
+    int iters_done[8];         // per level, copied from level_iter when the level ends
+    int pad1[56];
+};
+static_assert(sizeof(Control) == 512, "control block layout");
+
 // Where the three metrics of one warp_force pass go (S6 of the hot path).
 // Per-block partials in double, fixed-order final sum by the last block to finish: the result
-// does not depend on scheduling.
+// does not depend on scheduling.  Pair b of a batched launch uses ctl[b], partials + b * 5 * stride and
+// out + b * out_stride.
 struct MetricSink {
-    double* partials;           // [nvals][stride] block partials
-    unsigned int* ticket;       // block-completion counter, left at 0 by the last block
-    double* out;                // nullptr: metrics not wanted
-    unsigned int* row_counter;  // nullable: the last block writes out[3*row..] and bumps *row_counter
-    int stride;                 // capacity of one partial row (>= number of blocks)
-    // device-side stopping rule (reading A13); all nullable / eps <= 0 = off
-    double* lhist;              // ring of relative norms l_n for this level, [LHIST]
-    int* lvalid;                // l_n defined (sum|u| > 0), [LHIST]
-    unsigned int* level_iter;   // iterations executed on this level
-    int* stop_force;            // set to 1 when the rule fires; force kernels then skip
-    int* stop_smooth;           // set by the first skipped force kernel; smoothing then skips
-    double eps;
+    double* partials;   // [pairs][5][stride] block partials
+    Control* ctl;       // [pairs]
+    double* out;        // nullptr: metrics not wanted
+    size_t out_stride;  // doubles between the outputs of consecutive pairs
+    int stride;         // capacity of one partial row (>= number of blocks per pair)
+    int driver;         // 1 inside demons_register: rows advance, the stopping rule runs, stop flags are honoured
+    double eps;         // stopping rule threshold (<= 0: off)
 };
-
-constexpr int LHIST = 16;  // power of two >= 11 (lag of 10 iterations)
 
 __device__ __forceinline__ float lerpf(float a, float b, float t) { return fmaf(t, b - a, a); }
 
@@ -235,18 +247,17 @@ __device__ __forceinline__ double warp_max(double v) {
 }
 
 // Block-wide reduction of NV doubles (sum; the last NMAX of them by max), publication of the
-// block partial, and the fixed-order final reduction by the last block to arrive.  Returns true
-// in thread 0 of the last block, with the totals in v.  Must be called by every thread.
+// block partial, and the fixed-order final reduction by the last block to arrive (of the `nblocks` that
+// share this ticket; `bid` = this block's index among them).  Returns true in thread 0 of the last block,
+// with the totals in v.  Must be called by every thread.
 template <int NV, int NMAX = 0>
 __device__ __forceinline__ bool block_reduce_publish(double (&v)[NV], double* partials, int stride,
-                                                     unsigned int* ticket) {
+                                                     unsigned int* ticket, unsigned int bid, unsigned int nblocks) {
     __shared__ double sm[NV][32];
     __shared__ int s_last;
     const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
     const int nthreads = blockDim.x * blockDim.y * blockDim.z;
     const int lane = tid & 31, wid = tid >> 5, nwarps = (nthreads + 31) >> 5;
-    const unsigned int nblocks = gridDim.x * gridDim.y * gridDim.z;
-    const unsigned int bid = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
 #pragma unroll
     for (int i = 0; i < NV; ++i) {
         const double r = i >= NV - NMAX ? warp_max(v[i]) : warp_sum(v[i]);

@@ -40,25 +40,13 @@ int fail(int code, const char* fmt, ...) {
 constexpr size_t ALIGN = 256;
 size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
-// control block at the start of the workspace
-struct Control {
-    unsigned int ticket;       // 0
-    unsigned int row_counter;  // 4
-    unsigned int level_iter;   // 8
-    int stop_force;            // 12
-    int stop_smooth;           // 16
-    int pad0[11];              // -> 64
-    int lvalid[LHIST];         // 64
-    double lhist[LHIST];       // 128
-    int iters_done[DEMONS_MAX_LEVELS];  // 256
-    int pad1[56];
-};
-static_assert(sizeof(Control) == 512, "control block layout");
-
+// Workspace partition for `nb` pairs: every per-pair array is laid out [nb][...] so that one batched launch
+// covers a group of pairs.  The pyramid images of a pair are interleaved ([nb][2][n]: S then M), so that one L2
+// access-policy window covers the images of a group.
 struct Partition {
     size_t control, partials, stats, Mw, Sw, uprime, ubprime, smooth_tmp;
-    size_t pyrS[DEMONS_MAX_LEVELS], pyrM[DEMONS_MAX_LEVELS], pyrU[DEMONS_MAX_LEVELS], pyrUb[DEMONS_MAX_LEVELS];
-    size_t hS, hM, hU, hUb;
+    size_t pyrI[DEMONS_MAX_LEVELS], pyrU[DEMONS_MAX_LEVELS], pyrUb[DEMONS_MAX_LEVELS];
+    size_t hI, hU, hUb;
     size_t total;
     int partial_stride;
 };
@@ -67,7 +55,7 @@ struct GraphEntry {
     Dims d;
     const float *S, *M;
     float *u, *ub;
-    int chunk;
+    int chunk, nb, one_field;
     double eps;
     cudaGraphExec_t exec;
     int launches;
@@ -88,16 +76,12 @@ struct demons_ctx {
     int opt_texture = 0;
     int opt_generic_smooth = 0;
     int opt_profile = 0;
-    int opt_smooth_zc = 0;
-    int opt_no_tma = 0;
-    int opt_tune = 0;
     int opt_l2_persist = 1;
     int opt_zero_start = 0;
+    int opt_ic_one_field = 1;
     size_t l2_granted = 0;
     bool l2_limit_raised = false;
     size_t l2_prev_limit = 0;
-    int opt_force_zper = 0;
-    int opt_force_scalar = 0;
     std::vector<cudaEvent_t> prof_all;                               // events of the profiled call
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_pairs[4];  // per kernel class: start/stop
     double prof_ms[4] = {0, 0, 0, 0};
@@ -129,7 +113,7 @@ int gaussian_taps(double sigma, float* w) {
     return R;
 }
 
-Partition make_partition(const demons_ctx* c, int levels) {
+Partition make_partition(const demons_ctx* c, int levels, int nb) {
     Partition p{};
     const size_t N = nvox(c->dims);
     const bool ic = is_ic(c);
@@ -139,30 +123,30 @@ Partition make_partition(const demons_ctx* c, int levels) {
         off += align_up(bytes);
         return o;
     };
-    p.control = take(sizeof(Control));
+    p.control = take((size_t)nb * sizeof(Control));
     int stride = force_partial_blocks(c->dims);
     if (stride < 148 * 8) stride = 148 * 8;
     p.partial_stride = stride;
-    p.partials = take(5 * (size_t)stride * sizeof(double));  // 3 metrics per force block; 5 sums per block of demons_cc
-    p.stats = take((size_t)DEMONS_MAX_STATS_ROWS * 3 * sizeof(double));
-    p.Mw = take(N * 4);
-    p.Sw = ic ? take(N * 4) : 0;
-    p.uprime = take(3 * N * 4);
-    p.ubprime = ic ? take(3 * N * 4) : 0;
-    p.smooth_tmp = take(N * 4);
+    p.partials = take((size_t)nb * 5 * stride * sizeof(double));  // 3 metrics per force block; 5 sums per block of demons_cc
+    p.stats = take((size_t)nb * DEMONS_MAX_STATS_ROWS * 3 * sizeof(double));
+    p.Mw = take(nb * N * 4);
+    p.Sw = ic ? take(nb * N * 4) : 0;
+    p.uprime = take(nb * 3 * N * 4);
+    p.ubprime = ic ? take(nb * 3 * N * 4) : 0;
+    p.smooth_tmp = take(nb * N * 4);
     Dims d = c->dims;
     for (int l = 1; l < levels; ++l) {
         d = coarser(d);
         const size_t n = nvox(d);
-        p.pyrS[l] = take(n * 4);
-        p.pyrM[l] = take(n * 4);
-        p.pyrU[l] = take(3 * n * 4);
-        p.pyrUb[l] = ic ? take(3 * n * 4) : 0;
+        p.pyrI[l] = take(nb * 2 * n * 4);
+        p.pyrU[l] = take(nb * 3 * n * 4);
+        p.pyrUb[l] = ic ? take(nb * 3 * n * 4) : 0;
     }
-    p.hS = take(N * 4);
-    p.hM = take(N * 4);
-    p.hU = take(3 * N * 4);
-    p.hUb = ic ? take(3 * N * 4) : 0;
+    if (nb == 1) {  // staging of demons_register_host (single registrations only)
+        p.hI = take(2 * N * 4);
+        p.hU = take(3 * N * 4);
+        p.hUb = ic ? take(3 * N * 4) : 0;
+    }
     p.total = off;
     return p;
 }
@@ -175,12 +159,12 @@ bool dims_ok(const int dims[3]) {
     return n < 2147483647.0 / 4.0;
 }
 
-int check_ws(const demons_ctx* c, int levels) {
+int check_ws(const demons_ctx* c, int levels, int nb = 1) {
     if (!c->ws) return fail(DEMONS_E_WORKSPACE, "no workspace set (demons_set_workspace)");
-    const Partition p = make_partition(c, levels);
+    const Partition p = make_partition(c, levels, nb);
     if (p.total > c->ws_bytes)
-        return fail(DEMONS_E_WORKSPACE, "workspace too small: have %zu bytes, need %zu for %d level(s)",
-                    c->ws_bytes, p.total, levels);
+        return fail(DEMONS_E_WORKSPACE, "workspace too small: have %zu bytes, need %zu for %d level(s), batch of %d",
+                    c->ws_bytes, p.total, levels, nb);
     return DEMONS_OK;
 }
 
@@ -194,62 +178,82 @@ int check_call_dims(const demons_ctx* c, const int dims[3], Dims* out) {
     return DEMONS_OK;
 }
 
-// L2 residency for the gathered image (option "l2_persist", default on): raise the device's persisting-L2
-// set-aside (cudaLimitPersistingL2CacheSize, never lowered here) to the size of the moving image, capped by
-// the device maximum.  Returns the bytes the gathering kernels may ask to keep resident (0 = off).
-size_t persisting_l2_bytes(demons_ctx* c, const Dims& d, const float* S, const float* M) {
-    if (!c->opt_l2_persist) return 0;
-    static int max_persist = -1;
-    if (max_persist < 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        if (cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev) != cudaSuccess) {
-            cudaGetLastError();
-            max_persist = 0;
-        }
+// L2 residency for the gathered images (option "l2_persist", default on): the kernels that gather launch with an
+// access-policy window over the images of their group of pairs (hitProp = persisting).  The window is one
+// address range: [S_0, M_last] when the images of the group form one block (the workspace's pyramid levels do,
+// and so does a caller's pair whose moving image directly follows its static image), else the moving image of
+// a single pair.  The device's persisting-L2 set-aside (cudaLimitPersistingL2CacheSize) is RAISED to the size of
+// the window (never lowered here; demons_destroy restores it); windows larger than the device's maximum
+// set-aside are not requested at all: pinning a part of the images takes L2 away from everything else (the
+// smoothing halos, the stencils) and was 2x slower at 512x512x160.
+struct L2Window {
+    const void* ptr = nullptr;
+    size_t bytes = 0;
+    float ratio = 0.f;
+};
+
+bool images_form_block(const float* S, const float* M, size_t n, size_t img_stride, int nb) {
+    if (S == nullptr || M <= S) return false;
+    const size_t gap = (size_t)(M - S);
+    if (nb == 1) return gap <= n + 1024;            // M right behind S (at most one alignment gap)
+    return gap == n && img_stride == 2 * n;         // [nb][2][n]
+}
+
+L2Window l2_window(demons_ctx* c, const Dims& d, const float* S, const float* M, size_t img_stride, int nb) {
+    L2Window w;
+    if (!c->opt_l2_persist) return w;
+    const size_t max_persist = max_persisting_l2(), max_window = max_policy_window();
+    if (max_persist == 0 || max_window == 0) return w;
+    const size_t n = nvox(d);
+    const char* lo;
+    size_t span;
+    if (images_form_block(S, M, n, img_stride, nb)) {
+        lo = reinterpret_cast<const char*>(S);
+        span = (size_t)(reinterpret_cast<const char*>(M + (size_t)(nb - 1) * img_stride + n) - lo);
+    } else if (nb == 1) {
+        lo = reinterpret_cast<const char*>(M);
+        span = n * sizeof(float);
+    } else {
+        return w;
     }
-    if (max_persist <= 0) return 0;
-    // the window covers S as well when the moving image directly follows the static one in memory
-    // (the pyramid levels and the host-staging buffers of the workspace do; see launch_lc)
-    const size_t span = images_adjacent(S, M, nvox(d)) ? (size_t)((const char*)M - (const char*)S) + nvox(d) * 4 : nvox(d) * 4;
-    size_t want = (span + ((size_t)1 << 20) - 1) & ~(((size_t)1 << 20) - 1);
-    // Images that do not fit the set-aside whole are left alone: pinning a part of them takes L2 away from
-    // everything else (the smoothing halos, the stencils) and was 2x slower at 512x512x160.
-    if (want > (size_t)max_persist) return 0;
+    const size_t want = (span + ((size_t)1 << 20) - 1) & ~(((size_t)1 << 20) - 1);
+    if (want > max_persist || span > max_window) {
+        // both images of a pair do not fit: retry with the gathered (moving) image alone
+        if (nb == 1 && lo != reinterpret_cast<const char*>(M)) return l2_window(c, d, nullptr, M, img_stride, 1);
+        return w;
+    }
     size_t cur = 0;
     if (cudaDeviceGetLimit(&cur, cudaLimitPersistingL2CacheSize) != cudaSuccess) {
         cudaGetLastError();
-        return 0;
+        return w;
     }
     if (cur < want) {
         if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want) != cudaSuccess) {
             cudaGetLastError();
-            return 0;
+            return w;
         }
         if (!c->l2_limit_raised) {  // remember what to restore in demons_destroy
             c->l2_limit_raised = true;
             c->l2_prev_limit = cur;
         }
     }
-    return want;
+    c->l2_granted = want;
+    w.ptr = lo;
+    w.bytes = span;
+    w.ratio = 1.f;
+    return w;
 }
 
-MetricSink make_sink(const demons_ctx* c, const Partition& p, double* out, bool driver, double eps) {
+MetricSink make_sink(const demons_ctx* c, const Partition& p, int b0, double* out, size_t out_stride, bool driver,
+                     double eps) {
     MetricSink s{};
-    Control* ctl = reinterpret_cast<Control*>(c->ws + p.control);
-    s.partials = reinterpret_cast<double*>(c->ws + p.partials);
-    s.ticket = &ctl->ticket;
+    s.ctl = reinterpret_cast<Control*>(c->ws + p.control) + b0;
+    s.partials = reinterpret_cast<double*>(c->ws + p.partials) + (size_t)b0 * 5 * p.partial_stride;
     s.out = out;
+    s.out_stride = out_stride;
     s.stride = p.partial_stride;
-    if (driver) {
-        s.row_counter = &ctl->row_counter;
-        s.lhist = ctl->lhist;
-        s.lvalid = ctl->lvalid;
-        s.level_iter = &ctl->level_iter;
-        s.stop_force = &ctl->stop_force;
-        s.stop_smooth = &ctl->stop_smooth;
-        s.eps = eps;
-    }
+    s.driver = driver ? 1 : 0;
+    s.eps = eps;
     return s;
 }
 
@@ -326,39 +330,48 @@ void prof_collect(demons_ctx* c) {  // after a stream synchronise
 
 struct LevelBuffers {
     Dims d;
-    const float* S;
+    const float* S;     // pair 0 of the group
     const float* M;
-    float* u;
-    float* ub;
+    size_t img_stride;  // floats between the images of consecutive pairs
+    float* u;           // [nb][3][n]
+    float* ub;          // variant 5, two-field form; nullptr otherwise
+    int b0, nb;         // first pair and number of pairs of the group
+    int one_field;
 };
 
-// One iteration: [warp_force ; smooth the total field] (reading C2).
-int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb, double eps, cudaStream_t st,
-                      int* launches) {
+// One iteration of a group of pairs: [warp_force ; smooth the total field] (reading C2).
+int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb, const L2Window& win, double eps,
+                      cudaStream_t st, int* launches) {
     const bool ic = is_ic(c);
+    const bool two = ic && !lb.one_field;
+    const size_t N = nvox(c->dims);
     ForceArgs fa{};
     fa.d = lb.d;
     fa.variant = c->variant;
     fa.alpha2 = c->variant == DEMONS_ADJUSTED_DOUBLE ? c->alpha * c->alpha : 1.f;
+    fa.nb = lb.nb;
+    fa.img_stride = lb.img_stride;
     fa.S = lb.S;
     fa.M = lb.M;
     fa.u_in = lb.u;
-    fa.u_out = reinterpret_cast<float*>(c->ws + p.uprime);
-    fa.ub_in = ic ? lb.ub : nullptr;
-    fa.ub_out = ic ? reinterpret_cast<float*>(c->ws + p.ubprime) : nullptr;
-    fa.Mw = reinterpret_cast<float*>(c->ws + p.Mw);
-    fa.Sw = ic ? reinterpret_cast<float*>(c->ws + p.Sw) : nullptr;
-    fa.sink = make_sink(c, p, reinterpret_cast<double*>(c->ws + p.stats), true, eps);
+    // per-pair scratch is laid out for the level's own size, [nb][..n], starting at pair b0's share of the buffer
+    fa.u_out = reinterpret_cast<float*>(c->ws + p.uprime) + (size_t)lb.b0 * 3 * N;
+    fa.ub_in = two ? lb.ub : nullptr;
+    fa.ub_out = two ? reinterpret_cast<float*>(c->ws + p.ubprime) + (size_t)lb.b0 * 3 * N : nullptr;
+    fa.one_field = lb.one_field;
+    fa.Mw = reinterpret_cast<float*>(c->ws + p.Mw) + (size_t)lb.b0 * N;
+    fa.Sw = ic ? reinterpret_cast<float*>(c->ws + p.Sw) + (size_t)lb.b0 * N : nullptr;
+    fa.sink = make_sink(c, p, lb.b0, reinterpret_cast<double*>(c->ws + p.stats) + (size_t)lb.b0 * DEMONS_MAX_STATS_ROWS * 3,
+                        (size_t)DEMONS_MAX_STATS_ROWS * 3, true, eps);
     fa.texM = c->opt_texture ? c->tex : 0;
-    fa.zper = c->opt_force_zper;
-    fa.tune = c->opt_tune;
-    fa.l2_persist_bytes = c->l2_granted;  // set once per registration, outside any stream capture
-    fa.force_scalar = c->opt_force_scalar;
+    fa.l2_ptr = win.ptr;
+    fa.l2_bytes = win.bytes;
+    fa.l2_ratio = win.ratio;
     cudaEvent_t e0 = prof_event(c, st, true);
     fa.ev_mid = c->variant >= DEMONS_ACTIVE ? prof_event(c, st, false) : nullptr;
-    int n = launch_warp_force(fa, st);
-    if (n < 0) return fail(DEMONS_E_CUDA, "warp_force launch failed: %s", cudaGetErrorString(cudaGetLastError()));
-    *launches += n;
+    int k = launch_warp_force(fa, st);
+    if (k < 0) return fail(DEMONS_E_CUDA, "warp_force launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    *launches += k;
     cudaEvent_t e1 = prof_event(c, st, true);
     if (fa.ev_mid) {
         prof_pair(c, PROF_WARP, e0, fa.ev_mid);
@@ -368,25 +381,23 @@ int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb,
     }
     SmoothArgs sa{};
     sa.d = lb.d;
-    sa.tmp = reinterpret_cast<float*>(c->ws + p.smooth_tmp);
-    sa.ncomp = 3;
+    sa.tmp = reinterpret_cast<float*>(c->ws + p.smooth_tmp) + (size_t)lb.b0 * N;
+    sa.ncomp = 3 * lb.nb;
+    sa.comps_per_pair = 3;
     sa.R = gaussian_taps(c->sigma, sa.w);
-    sa.skip = &reinterpret_cast<Control*>(c->ws + p.control)->stop_smooth;
+    sa.ctl = reinterpret_cast<Control*>(c->ws + p.control) + lb.b0;
     sa.force_generic = c->opt_generic_smooth;
-    sa.zc_override = c->opt_smooth_zc;
-    sa.no_tma = c->opt_no_tma;
-    sa.tune = c->opt_tune;
     sa.in = fa.u_out;
     sa.out = lb.u;
-    n = launch_smooth(sa, st);
-    if (n < 0) return fail(DEMONS_E_CUDA, "smooth launch failed: %s", cudaGetErrorString(cudaGetLastError()));
-    *launches += n;
-    if (ic) {
+    k = launch_smooth(sa, st);
+    if (k < 0) return fail(DEMONS_E_CUDA, "smooth launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    *launches += k;
+    if (two) {
         sa.in = fa.ub_out;
         sa.out = lb.ub;
-        n = launch_smooth(sa, st);
-        if (n < 0) return fail(DEMONS_E_CUDA, "smooth launch failed: %s", cudaGetErrorString(cudaGetLastError()));
-        *launches += n;
+        k = launch_smooth(sa, st);
+        if (k < 0) return fail(DEMONS_E_CUDA, "smooth launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        *launches += k;
     }
     prof_pair(c, PROF_SMOOTH, e1, prof_event(c, st, true));
     return DEMONS_OK;
@@ -394,10 +405,14 @@ int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb,
 
 bool capturable(cudaStream_t st) { return st != nullptr && st != cudaStreamLegacy; }
 
+constexpr size_t GRAPH_CACHE = 192;
+
 int run_level(demons_ctx* c, const Partition& p, const LevelBuffers& lb, int iters, double eps, cudaStream_t st) {
     int done = 0;
+    const size_t N = nvox(c->dims);
+    const L2Window win = l2_window(c, lb.d, lb.S, lb.M, lb.img_stride, lb.nb);  // outside any stream capture
     if (c->variant == DEMONS_EVOLVED_PASSIVE && iters > 0) {  // |grad M0|^2 of this level, fixed for the level
-        if (launch_grad_mag2(lb.d, lb.M, reinterpret_cast<float*>(c->ws + p.Mw), st) < 0)
+        if (launch_grad_mag2(lb.d, lb.M, lb.img_stride, reinterpret_cast<float*>(c->ws + p.Mw) + (size_t)lb.b0 * N, lb.nb, st) < 0)
             return fail(DEMONS_E_CUDA, "gradient launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         c->launches += 1;
     }
@@ -406,7 +421,8 @@ int run_level(demons_ctx* c, const Partition& p, const LevelBuffers& lb, int ite
         GraphEntry* ge = nullptr;
         for (auto& g : c->graphs)
             if (g.d.nx == lb.d.nx && g.d.ny == lb.d.ny && g.d.nz == lb.d.nz && g.S == lb.S && g.M == lb.M &&
-                g.u == lb.u && g.ub == lb.ub && g.chunk == chunk && g.eps == eps)
+                g.u == lb.u && g.ub == lb.ub && g.chunk == chunk && g.eps == eps && g.nb == lb.nb &&
+                g.one_field == lb.one_field)
                 ge = &g;
         if (!ge) {
             GraphEntry g{};
@@ -417,10 +433,12 @@ int run_level(demons_ctx* c, const Partition& p, const LevelBuffers& lb, int ite
             g.ub = lb.ub;
             g.chunk = chunk;
             g.eps = eps;
+            g.nb = lb.nb;
+            g.one_field = lb.one_field;
             cudaGraph_t graph = nullptr;
             CUDA_TRY(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
             int rc = DEMONS_OK;
-            for (int i = 0; i < chunk && rc == DEMONS_OK; ++i) rc = enqueue_iteration(c, p, lb, eps, st, &g.launches);
+            for (int i = 0; i < chunk && rc == DEMONS_OK; ++i) rc = enqueue_iteration(c, p, lb, win, eps, st, &g.launches);
             cudaError_t e = cudaStreamEndCapture(st, &graph);
             if (rc != DEMONS_OK) {
                 if (graph) cudaGraphDestroy(graph);
@@ -430,7 +448,7 @@ int run_level(demons_ctx* c, const Partition& p, const LevelBuffers& lb, int ite
             e = cudaGraphInstantiate(&g.exec, graph, 0);
             cudaGraphDestroy(graph);
             if (e != cudaSuccess) return fail(DEMONS_E_CUDA, "graph instantiate failed: %s", cudaGetErrorString(e));
-            if (c->graphs.size() >= 32) {  // bounded cache
+            if (c->graphs.size() >= GRAPH_CACHE) {  // bounded cache
                 cudaGraphExecDestroy(c->graphs.front().exec);
                 c->graphs.erase(c->graphs.begin());
             }
@@ -444,85 +462,137 @@ int run_level(demons_ctx* c, const Partition& p, const LevelBuffers& lb, int ite
         }
     }
     for (; done < iters; ++done) {
-        int n = 0;
-        const int rc = enqueue_iteration(c, p, lb, eps, st, &n);
+        int k = 0;
+        const int rc = enqueue_iteration(c, p, lb, win, eps, st, &k);
         if (rc != DEMONS_OK) return rc;
-        c->launches += n;
+        c->launches += k;
     }
     return DEMONS_OK;
 }
 
-int register_impl(demons_ctx* c, const float* dS, const float* dM, float* du, float* dub, int levels,
+// Pairs per launch on a level of n voxels: enough voxels per launch to fill the GPU (a 256x256x100 level
+// does; a 64x64x25 level needs the whole batch), never more than the batch.  Large levels run pair by pair:
+// their launches already fill the machine and the images of ONE pair stay resident in L2.
+int group_size(size_t n, int nb) {
+    const size_t target = (size_t)3 << 20;  // voxels per launch
+    size_t g = (target + n - 1) / n;
+    if (g < 1) g = 1;
+    if (g > (size_t)nb) g = nb;
+    return (int)g;
+}
+
+// The multi-scale driver (O9) for a batch of nb independent pairs: images [nb][N], fields [nb][3][N].
+int register_impl(demons_ctx* c, const float* dS, const float* dM, float* du, float* dub, int nb, int levels,
                   const int* iters, double eps, double* h_stats, int* h_done, cudaStream_t st) {
     const bool ic = is_ic(c);
-    const Partition p = make_partition(c, levels);
-    c->l2_granted = persisting_l2_bytes(c, c->dims, dS, dM);
+    const Partition p = make_partition(c, levels, nb);
+    const size_t N = nvox(c->dims);
     Control* ctl = reinterpret_cast<Control*>(c->ws + p.control);
     long long total_iters = 0;
     for (int l = 0; l < levels; ++l) total_iters += iters[l];
+    const bool zero_start = levels > 1 || c->opt_zero_start;
+    // variant 5 from a zero start: u_b = -u_f exactly at every iteration and level (pin P10), so only u_f is
+    // iterated on and u_b is written once on exit; bit-identical to iterating on both fields
+    const int one_field = ic && zero_start && c->opt_ic_one_field ? 1 : 0;
     prof_clear(c);
-    CUDA_TRY(cudaMemsetAsync(ctl, 0, sizeof(Control), st));
-    if (total_iters > 0) CUDA_TRY(cudaMemsetAsync(c->ws + p.stats, 0, (size_t)total_iters * 24, st));
+    CUDA_TRY(cudaMemsetAsync(ctl, 0, (size_t)nb * sizeof(Control), st));
+    if (total_iters > 0)
+        CUDA_TRY(cudaMemsetAsync(c->ws + p.stats, 0,
+                                 ((size_t)(nb - 1) * DEMONS_MAX_STATS_ROWS + (size_t)total_iters) * 24, st));
 
     // pyramids (O6): images only, no pre-blur (reading A15)
-    LevelBuffers lb[DEMONS_MAX_LEVELS];
-    lb[0] = LevelBuffers{c->dims, dS, dM, du, dub};
+    struct Level {
+        Dims d;
+        const float *S, *M;
+        size_t img_stride;
+        float *u, *ub;
+    } lv[DEMONS_MAX_LEVELS];
+    lv[0] = Level{c->dims, dS, dM, N, du, dub};  // the caller's layout: static [nb][N], moving [nb][N]
     for (int l = 1; l < levels; ++l) {
-        lb[l].d = coarser(lb[l - 1].d);
-        float* s = reinterpret_cast<float*>(c->ws + p.pyrS[l]);
-        float* m = reinterpret_cast<float*>(c->ws + p.pyrM[l]);
-        lb[l].S = s;
-        lb[l].M = m;
-        lb[l].u = reinterpret_cast<float*>(c->ws + p.pyrU[l]);
-        lb[l].ub = ic ? reinterpret_cast<float*>(c->ws + p.pyrUb[l]) : nullptr;
+        lv[l].d = coarser(lv[l - 1].d);
+        const size_t n = nvox(lv[l].d);
+        float* base = reinterpret_cast<float*>(c->ws + p.pyrI[l]);
+        lv[l].S = base;
+        lv[l].M = base + n;
+        lv[l].img_stride = 2 * n;
+        lv[l].u = reinterpret_cast<float*>(c->ws + p.pyrU[l]);
+        lv[l].ub = ic ? reinterpret_cast<float*>(c->ws + p.pyrUb[l]) : nullptr;
         cudaEvent_t e0 = prof_event(c, st, true);
-        if (launch_restrict(lb[l - 1].d, lb[l - 1].S, s, st) < 0 || launch_restrict(lb[l - 1].d, lb[l - 1].M, m, st) < 0)
+        if (launch_restrict(lv[l - 1].d, lv[l - 1].S, lv[l - 1].img_stride, base, 2 * n, nb, st) < 0 ||
+            launch_restrict(lv[l - 1].d, lv[l - 1].M, lv[l - 1].img_stride, base + n, 2 * n, nb, st) < 0)
             return fail(DEMONS_E_CUDA, "restrict launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         c->launches += 2;
         prof_pair(c, PROF_PYRAMID, e0, prof_event(c, st, true));
     }
-    if (levels > 1 || c->opt_zero_start) {  // the coarsest level starts from zero (O9); "zero_start": a single level too
-        const size_t n = nvox(lb[levels - 1].d);
-        CUDA_TRY(cudaMemsetAsync(lb[levels - 1].u, 0, 3 * n * 4, st));
-        if (ic) CUDA_TRY(cudaMemsetAsync(lb[levels - 1].ub, 0, 3 * n * 4, st));
+    if (zero_start) {  // the coarsest level starts from zero (O9); "zero_start": a single level too
+        const size_t n = nvox(lv[levels - 1].d);
+        CUDA_TRY(cudaMemsetAsync(lv[levels - 1].u, 0, (size_t)nb * 3 * n * 4, st));
+        if (ic && !one_field) CUDA_TRY(cudaMemsetAsync(lv[levels - 1].ub, 0, (size_t)nb * 3 * n * 4, st));
     }
     for (int step = 0; step < levels; ++step) {
         const int l = levels - 1 - step;  // coarse -> fine
-        if (step > 0) CUDA_TRY(cudaMemsetAsync(&ctl->level_iter, 0, 12, st));  // level_iter, stop_force, stop_smooth
-        if (c->opt_texture) {
-            const int rc = bind_texture(c, lb[l].d, lb[l].M, st);
+        const size_t n = nvox(lv[l].d);
+        const int G = group_size(n, nb);
+        if (step > 0)  // level_iter, stop_force, stop_smooth of every pair
+            CUDA_TRY(cudaMemset2DAsync(&ctl[0].level_iter, sizeof(Control), 0, 12, nb, st));
+        for (int b0 = 0; b0 < nb; b0 += G) {
+            const int g = nb - b0 < G ? nb - b0 : G;
+            LevelBuffers lb{};
+            lb.d = lv[l].d;
+            lb.S = lv[l].S + (size_t)b0 * lv[l].img_stride;
+            lb.M = lv[l].M + (size_t)b0 * lv[l].img_stride;
+            lb.img_stride = lv[l].img_stride;
+            lb.u = lv[l].u + (size_t)b0 * 3 * n;
+            lb.ub = ic && !one_field ? lv[l].ub + (size_t)b0 * 3 * n : nullptr;
+            lb.b0 = b0;
+            lb.nb = g;
+            lb.one_field = one_field;
+            if (c->opt_texture) {
+                const int rc = bind_texture(c, lb.d, lb.M, st);
+                if (rc != DEMONS_OK) return rc;
+            }
+            const int rc = run_level(c, p, lb, iters[step], eps, st);
             if (rc != DEMONS_OK) return rc;
-        }
-        const int rc = run_level(c, p, lb[l], iters[step], eps, st);
-        if (rc != DEMONS_OK) return rc;
-        CUDA_TRY(cudaMemcpyAsync(&ctl->iters_done[step], &ctl->level_iter, 4, cudaMemcpyDeviceToDevice, st));
-        if (l > 0) {  // O7
-            cudaEvent_t e0 = prof_event(c, st, true);
-            if (launch_prolong(lb[l].d, lb[l].u, lb[l - 1].d, lb[l - 1].u, st) < 0)
-                return fail(DEMONS_E_CUDA, "prolong launch failed: %s", cudaGetErrorString(cudaGetLastError()));
-            c->launches += 1;
-            if (ic) {
-                if (launch_prolong(lb[l].d, lb[l].ub, lb[l - 1].d, lb[l - 1].ub, st) < 0)
+            if (l > 0) {  // O7
+                const size_t nf = nvox(lv[l - 1].d);
+                cudaEvent_t e0 = prof_event(c, st, true);
+                if (launch_prolong(lb.d, lb.u, lv[l - 1].d, lv[l - 1].u + (size_t)b0 * 3 * nf, g, st) < 0)
                     return fail(DEMONS_E_CUDA, "prolong launch failed: %s", cudaGetErrorString(cudaGetLastError()));
                 c->launches += 1;
+                if (ic && !one_field) {
+                    if (launch_prolong(lb.d, lb.ub, lv[l - 1].d, lv[l - 1].ub + (size_t)b0 * 3 * nf, g, st) < 0)
+                        return fail(DEMONS_E_CUDA, "prolong launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+                    c->launches += 1;
+                }
+                prof_pair(c, PROF_PYRAMID, e0, prof_event(c, st, true));
             }
-            prof_pair(c, PROF_PYRAMID, e0, prof_event(c, st, true));
         }
+        CUDA_TRY(cudaMemcpy2DAsync(&ctl[0].iters_done[step], sizeof(Control), &ctl[0].level_iter, sizeof(Control), 4, nb,
+                                   cudaMemcpyDeviceToDevice, st));
+    }
+    if (one_field) {  // u_b = -u_f (P10), written once
+        if (launch_negate(du, dub, (size_t)nb * 3 * N, st) < 0)
+            return fail(DEMONS_E_CUDA, "negate launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        c->launches += 1;
     }
     if (h_stats && total_iters > 0)
-        CUDA_TRY(cudaMemcpyAsync(h_stats, c->ws + p.stats, (size_t)total_iters * 24, cudaMemcpyDeviceToHost, st));
-    if (h_done) CUDA_TRY(cudaMemcpyAsync(h_done, ctl->iters_done, (size_t)levels * 4, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaMemcpy2DAsync(h_stats, (size_t)total_iters * 24, c->ws + p.stats, (size_t)DEMONS_MAX_STATS_ROWS * 24,
+                                   (size_t)total_iters * 24, nb, cudaMemcpyDeviceToHost, st));
+    if (h_done)
+        CUDA_TRY(cudaMemcpy2DAsync(h_done, (size_t)levels * 4, ctl[0].iters_done, sizeof(Control), (size_t)levels * 4, nb,
+                                   cudaMemcpyDeviceToHost, st));
     if (h_stats || h_done || c->opt_profile) CUDA_TRY(cudaStreamSynchronize(st));
     if (c->opt_profile) prof_collect(c);
     return DEMONS_OK;
 }
 
-int check_register_args(demons_ctx* c, const void* S, const void* M, const void* u, const void* ub, int levels,
+int check_register_args(demons_ctx* c, const void* S, const void* M, const void* u, const void* ub, int nb, int levels,
                         const int* iters) {
     if (!c) return fail(DEMONS_E_ARG, "ctx is NULL");
     if (!S || !M || !u) return fail(DEMONS_E_ARG, "static, moving and u must be non-NULL");
     if (is_ic(c) && !ub) return fail(DEMONS_E_ARG, "variant 5 needs u_back");
     if (!is_ic(c) && ub) return fail(DEMONS_E_ARG, "u_back must be NULL unless variant 5");
+    if (nb < 1 || nb > DEMONS_MAX_BATCH) return fail(DEMONS_E_ARG, "batch size out of range");
     if (levels < 1 || levels > DEMONS_MAX_LEVELS) return fail(DEMONS_E_ARG, "levels out of range");
     if (!iters) return fail(DEMONS_E_ARG, "iters_per_level is NULL");
     long long total = 0;
@@ -531,7 +601,10 @@ int check_register_args(demons_ctx* c, const void* S, const void* M, const void*
         total += iters[l];
     }
     if (total > DEMONS_MAX_STATS_ROWS) return fail(DEMONS_E_ARG, "more than DEMONS_MAX_STATS_ROWS iterations");
-    return check_ws(c, levels);
+    if (nb > 1 && c->opt_texture) return fail(DEMONS_E_UNSUPPORTED, "the texture option serves single registrations only");
+    if (nb > 1 && (double)nb * (double)nvox(c->dims) >= 2147483647.0 / 4.0 && group_size(nvox(c->dims), nb) > 1)
+        return fail(DEMONS_E_UNSUPPORTED, "batch too large for 32-bit indexing");
+    return check_ws(c, levels, nb);
 }
 
 }  // namespace
@@ -581,14 +654,20 @@ void demons_destroy(demons_ctx* c) {
 
 size_t demons_workspace_bytes(const demons_ctx* c, int levels) {
     if (!c || levels < 1 || levels > DEMONS_MAX_LEVELS) return 0;
-    return make_partition(c, levels).total;
+    return make_partition(c, levels, 1).total;
+}
+
+size_t demons_workspace_bytes_batch(const demons_ctx* c, int levels, int nbatch) {
+    if (!c || levels < 1 || levels > DEMONS_MAX_LEVELS || nbatch < 1 || nbatch > DEMONS_MAX_BATCH) return 0;
+    const size_t single = make_partition(c, levels, 1).total, batch = make_partition(c, levels, nbatch).total;
+    return batch > single ? batch : single;  // every single-registration entry point keeps working
 }
 
 int demons_set_workspace(demons_ctx* c, void* d_ws, size_t bytes) {
     if (!c || !d_ws) return fail(DEMONS_E_ARG, "ctx / workspace is NULL");
     if (reinterpret_cast<uintptr_t>(d_ws) % ALIGN) return fail(DEMONS_E_ARG, "workspace must be 256-byte aligned");
-    if (bytes < make_partition(c, 1).total)
-        return fail(DEMONS_E_WORKSPACE, "workspace too small: %zu < %zu", bytes, make_partition(c, 1).total);
+    if (bytes < make_partition(c, 1, 1).total)
+        return fail(DEMONS_E_WORKSPACE, "workspace too small: %zu < %zu", bytes, make_partition(c, 1, 1).total);
     for (auto& g : c->graphs) cudaGraphExecDestroy(g.exec);
     c->graphs.clear();
     CUDA_TRY(cudaMemset(d_ws, 0, sizeof(Control)));
@@ -625,13 +704,9 @@ int demons_set_option(demons_ctx* c, const char* name, int value) {
     else if (!strcmp(name, "texture")) c->opt_texture = value != 0;
     else if (!strcmp(name, "generic_smooth")) c->opt_generic_smooth = value != 0;
     else if (!strcmp(name, "profile")) c->opt_profile = value != 0;
-    else if (!strcmp(name, "smooth_zc")) c->opt_smooth_zc = value;
-    else if (!strcmp(name, "no_tma")) c->opt_no_tma = value != 0;
-    else if (!strcmp(name, "tune")) c->opt_tune = value;
     else if (!strcmp(name, "l2_persist")) c->opt_l2_persist = value != 0;
     else if (!strcmp(name, "zero_start")) c->opt_zero_start = value != 0;
-    else if (!strcmp(name, "force_zper")) c->opt_force_zper = value;
-    else if (!strcmp(name, "force_scalar")) c->opt_force_scalar = value != 0;
+    else if (!strcmp(name, "ic_one_field")) c->opt_ic_one_field = value != 0;
     else return fail(DEMONS_E_ARG, "unknown option '%s'", name);
     for (auto& g : c->graphs) cudaGraphExecDestroy(g.exec);
     c->graphs.clear();
@@ -640,23 +715,32 @@ int demons_set_option(demons_ctx* c, const char* name, int value) {
 
 int demons_register(demons_ctx* c, const float* d_static, const float* d_moving, float* d_u, float* d_u_back,
                     int levels, const int* h_iters, double eps, double* h_stats, int* h_iters_done, void* stream) {
-    const int rc = check_register_args(c, d_static, d_moving, d_u, d_u_back, levels, h_iters);
+    const int rc = check_register_args(c, d_static, d_moving, d_u, d_u_back, 1, levels, h_iters);
     if (rc != DEMONS_OK) return rc;
-    return register_impl(c, d_static, d_moving, d_u, d_u_back, levels, h_iters, eps, h_stats, h_iters_done,
+    return register_impl(c, d_static, d_moving, d_u, d_u_back, 1, levels, h_iters, eps, h_stats, h_iters_done,
+                         static_cast<cudaStream_t>(stream));
+}
+
+int demons_register_batch(demons_ctx* c, int nbatch, const float* d_static, const float* d_moving, float* d_u,
+                          float* d_u_back, int levels, const int* h_iters, double eps, double* h_stats,
+                          int* h_iters_done, void* stream) {
+    const int rc = check_register_args(c, d_static, d_moving, d_u, d_u_back, nbatch, levels, h_iters);
+    if (rc != DEMONS_OK) return rc;
+    return register_impl(c, d_static, d_moving, d_u, d_u_back, nbatch, levels, h_iters, eps, h_stats, h_iters_done,
                          static_cast<cudaStream_t>(stream));
 }
 
 int demons_register_host(demons_ctx* c, const float* h_static, const float* h_moving, float* h_u, float* h_u_back,
                          int levels, const int* h_iters, double eps, double* h_stats, int* h_iters_done,
                          void* stream) {
-    const int rc = check_register_args(c, h_static, h_moving, h_u, h_u_back, levels, h_iters);
+    const int rc = check_register_args(c, h_static, h_moving, h_u, h_u_back, 1, levels, h_iters);
     if (rc != DEMONS_OK) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const Partition p = make_partition(c, levels);
+    const Partition p = make_partition(c, levels, 1);
     const size_t N = nvox(c->dims);
     const bool ic = is_ic(c);
-    float* dS = reinterpret_cast<float*>(c->ws + p.hS);
-    float* dM = reinterpret_cast<float*>(c->ws + p.hM);
+    float* dS = reinterpret_cast<float*>(c->ws + p.hI);  // M right behind S: one L2 window covers both
+    float* dM = dS + N;
     float* dU = reinterpret_cast<float*>(c->ws + p.hU);
     float* dUb = ic ? reinterpret_cast<float*>(c->ws + p.hUb) : nullptr;
     CUDA_TRY(cudaMemcpyAsync(dS, h_static, N * 4, cudaMemcpyHostToDevice, st));
@@ -665,7 +749,7 @@ int demons_register_host(demons_ctx* c, const float* h_static, const float* h_mo
         CUDA_TRY(cudaMemcpyAsync(dU, h_u, 3 * N * 4, cudaMemcpyHostToDevice, st));
         if (ic) CUDA_TRY(cudaMemcpyAsync(dUb, h_u_back, 3 * N * 4, cudaMemcpyHostToDevice, st));
     }
-    const int rr = register_impl(c, dS, dM, dU, dUb, levels, h_iters, eps, nullptr, nullptr, st);
+    const int rr = register_impl(c, dS, dM, dU, dUb, 1, levels, h_iters, eps, nullptr, nullptr, st);
     if (rr != DEMONS_OK) return rr;
     CUDA_TRY(cudaMemcpyAsync(h_u, dU, 3 * N * 4, cudaMemcpyDeviceToHost, st));
     if (ic) CUDA_TRY(cudaMemcpyAsync(h_u_back, dUb, 3 * N * 4, cudaMemcpyDeviceToHost, st));
@@ -696,11 +780,13 @@ int demons_warp_force(demons_ctx* c, const int dims[3], const float* d_static, c
     rc = check_ws(c, 1);
     if (rc != DEMONS_OK) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const Partition p = make_partition(c, 1);
+    const Partition p = make_partition(c, 1, 1);
     ForceArgs fa{};
     fa.d = d;
     fa.variant = c->variant;
     fa.alpha2 = c->variant == DEMONS_ADJUSTED_DOUBLE ? c->alpha * c->alpha : 1.f;
+    fa.nb = 1;
+    fa.img_stride = nvox(d);
     fa.S = d_static;
     fa.M = d_moving;
     fa.u_in = d_u_in;
@@ -709,18 +795,18 @@ int demons_warp_force(demons_ctx* c, const int dims[3], const float* d_static, c
     fa.ub_out = d_ub_out;
     fa.Mw = reinterpret_cast<float*>(c->ws + p.Mw);
     fa.Sw = ic ? reinterpret_cast<float*>(c->ws + p.Sw) : nullptr;
-    fa.sink = make_sink(c, p, d_metrics, false, 0.0);
-    fa.zper = c->opt_force_zper;
-    fa.tune = c->opt_tune;
-    fa.l2_persist_bytes = c->l2_granted = persisting_l2_bytes(c, fa.d, d_static, d_moving);
-    fa.force_scalar = c->opt_force_scalar;
+    fa.sink = make_sink(c, p, 0, d_metrics, 0, false, 0.0);
+    const L2Window win = l2_window(c, d, d_static, d_moving, nvox(d), 1);
+    fa.l2_ptr = win.ptr;
+    fa.l2_bytes = win.bytes;
+    fa.l2_ratio = win.ratio;
     if (c->opt_texture) {
         rc = bind_texture(c, d, d_moving, st);
         if (rc != DEMONS_OK) return rc;
         fa.texM = c->tex;
     }
     if (c->variant == DEMONS_EVOLVED_PASSIVE) {
-        if (launch_grad_mag2(d, d_moving, fa.Mw, st) < 0)
+        if (launch_grad_mag2(d, d_moving, nvox(d), fa.Mw, 1, st) < 0)
             return fail(DEMONS_E_CUDA, "gradient launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         c->launches += 1;
     }
@@ -745,17 +831,15 @@ int demons_smooth(demons_ctx* c, const int dims[3], const float* d_in, float* d_
     if (sa.R < 0) return fail(DEMONS_E_UNSUPPORTED, "ceil(3 sigma) exceeds DEMONS_MAX_RADIUS (%d)", DEMONS_MAX_RADIUS);
     rc = check_ws(c, 1);
     if (rc != DEMONS_OK) return rc;
-    const Partition p = make_partition(c, 1);
+    const Partition p = make_partition(c, 1, 1);
     sa.d = d;
     sa.in = d_in;
     sa.out = d_out;
     sa.tmp = reinterpret_cast<float*>(c->ws + p.smooth_tmp);
     sa.ncomp = ncomp;
-    sa.skip = nullptr;
+    sa.comps_per_pair = ncomp;
+    sa.ctl = nullptr;
     sa.force_generic = c->opt_generic_smooth;
-    sa.zc_override = c->opt_smooth_zc;
-    sa.no_tma = c->opt_no_tma;
-    sa.tune = c->opt_tune;
     const int n = launch_smooth(sa, static_cast<cudaStream_t>(stream));
     if (n < 0) return fail(DEMONS_E_CUDA, "smooth launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     c->launches += n;
@@ -767,7 +851,7 @@ int demons_restrict(demons_ctx* c, const int fine_dims[3], const float* d_fine, 
     if (!dims_ok(fine_dims)) return fail(DEMONS_E_ARG, "bad dims");
     if (!d_fine || !d_coarse) return fail(DEMONS_E_ARG, "NULL volume pointer");
     const Dims fd{fine_dims[0], fine_dims[1], fine_dims[2]};
-    if (launch_restrict(fd, d_fine, d_coarse, static_cast<cudaStream_t>(stream)) < 0)
+    if (launch_restrict(fd, d_fine, 0, d_coarse, 0, 1, static_cast<cudaStream_t>(stream)) < 0)
         return fail(DEMONS_E_CUDA, "restrict launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     c->launches += 1;
     return DEMONS_OK;
@@ -783,7 +867,7 @@ int demons_prolong(demons_ctx* c, const int coarse_dims[3], const float* d_uc, c
             return fail(DEMONS_E_ARG, "coarse dims must be ceil(fine dims / 2)");
     const Dims cd{coarse_dims[0], coarse_dims[1], coarse_dims[2]};
     const Dims fd{fine_dims[0], fine_dims[1], fine_dims[2]};
-    if (launch_prolong(cd, d_uc, fd, d_uf, static_cast<cudaStream_t>(stream)) < 0)
+    if (launch_prolong(cd, d_uc, fd, d_uf, 1, static_cast<cudaStream_t>(stream)) < 0)
         return fail(DEMONS_E_CUDA, "prolong launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     c->launches += 1;
     return DEMONS_OK;
@@ -799,7 +883,7 @@ int demons_ssd(demons_ctx* c, const int dims[3], const float* d_static, const fl
     if (is_ic(c) != (d_ub != nullptr)) return fail(DEMONS_E_ARG, "ub must be given exactly for variant 5");
     rc = check_ws(c, 1);
     if (rc != DEMONS_OK) return rc;
-    const Partition p = make_partition(c, 1);
+    const Partition p = make_partition(c, 1, 1);
     ReduceScratch rs{reinterpret_cast<double*>(c->ws + p.partials),
                      &reinterpret_cast<Control*>(c->ws + p.control)->ticket, p.partial_stride};
     if (launch_ssd(d, d_static, d_moving, d_u, d_ub, d_out, rs, static_cast<cudaStream_t>(stream)) < 0)
@@ -817,7 +901,7 @@ int demons_ic_error(demons_ctx* c, const int dims[3], const float* d_uf, const f
     if (!d_uf || !d_ub || !d_out) return fail(DEMONS_E_ARG, "NULL pointer");
     rc = check_ws(c, 1);
     if (rc != DEMONS_OK) return rc;
-    const Partition p = make_partition(c, 1);
+    const Partition p = make_partition(c, 1, 1);
     ReduceScratch rs{reinterpret_cast<double*>(c->ws + p.partials),
                      &reinterpret_cast<Control*>(c->ws + p.control)->ticket, p.partial_stride};
     if (launch_ic_error(d, d_uf, d_ub, d_out, rs, static_cast<cudaStream_t>(stream)) < 0)
@@ -837,7 +921,7 @@ int demons_cc(demons_ctx* c, const int dims[3], const float* d_static, const flo
     if (!is_ic(c) && d_ub) return fail(DEMONS_E_ARG, "u_back must be NULL unless variant 5");
     rc = check_ws(c, 1);
     if (rc != DEMONS_OK) return rc;
-    const Partition p = make_partition(c, 1);
+    const Partition p = make_partition(c, 1, 1);
     ReduceScratch rs{reinterpret_cast<double*>(c->ws + p.partials),
                      &reinterpret_cast<Control*>(c->ws + p.control)->ticket, p.partial_stride};
     if (launch_cc(d, d_static, d_moving, d_u, d_ub, d_out, rs, static_cast<cudaStream_t>(stream)) < 0)

@@ -9,12 +9,16 @@ namespace {
 
 // O6: coarse(i,j,k) = mean of the 2x2x2 fine voxels {2i, min(2i+1, n-1)} x ...; n_c = ceil(n_f/2)
 // (2x2x2 averaging per BASELINE.json config 3; odd tail counted twice, reading A12).
+// blockIdx.z = pair * cd.nz + k (a batch of images in one launch).
 __global__ void __launch_bounds__(256) k_restrict(const float* __restrict__ fine, float* __restrict__ coarse,
-                                                  const Dims fd, const Dims cd) {
+                                                  const Dims fd, const Dims cd, const size_t in_stride,
+                                                  const size_t out_stride) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
-    const int k = blockIdx.z;
+    const int pair = blockIdx.z / cd.nz, k = blockIdx.z - pair * cd.nz;
     if (i >= cd.nx || j >= cd.ny) return;
+    fine += (size_t)pair * in_stride;
+    coarse += (size_t)pair * out_stride;
     const int x0 = 2 * i, x1 = min(2 * i + 1, fd.nx - 1);
     const int y0 = 2 * j, y1 = min(2 * j + 1, fd.ny - 1);
     const int z0 = 2 * k, z1 = min(2 * k + 1, fd.nz - 1);
@@ -39,8 +43,11 @@ __global__ void __launch_bounds__(256) k_prolong(const float* __restrict__ uc, f
                                                  const Dims cd, const Dims fd) {
     const int i = (int)(blockIdx.x * blockDim.x + threadIdx.x) - 1;
     const int j = (int)(blockIdx.y * blockDim.y + threadIdx.y) - 1;
-    const int k = (int)blockIdx.z - 1;
+    const int b = blockIdx.z / (cd.nz + 1);  // blockIdx.z = pair * (cd.nz + 1) + (k + 1)
+    const int k = (int)(blockIdx.z - b * (cd.nz + 1)) - 1;
     if (i >= cd.nx || j >= cd.ny) return;
+    uc += (size_t)b * 3 * nvox(cd);
+    uf += (size_t)b * 3 * nvox(fd);
     const int x0 = max(i, 0), x1 = min(i + 1, cd.nx - 1);
     const int y0 = max(j, 0), y1 = min(j + 1, cd.ny - 1);
     const int z0 = max(k, 0), z1 = min(k + 1, cd.nz - 1);
@@ -80,17 +87,20 @@ __global__ void __launch_bounds__(256) k_prolong(const float* __restrict__ uc, f
 
 }  // namespace
 
-int launch_restrict(const Dims& fd, const float* in, float* out, cudaStream_t st) {
+int launch_restrict(const Dims& fd, const float* in, size_t in_stride, float* out, size_t out_stride, int nb,
+                    cudaStream_t st) {
     const Dims cd{(fd.nx + 1) / 2, (fd.ny + 1) / 2, (fd.nz + 1) / 2};
+    if ((long long)cd.nz * nb > 65535) return -1;
     const dim3 block(64, 4);
-    const dim3 grid((cd.nx + 63) / 64, (cd.ny + 3) / 4, cd.nz);
-    k_restrict<<<grid, block, 0, st>>>(in, out, fd, cd);
+    const dim3 grid((cd.nx + 63) / 64, (cd.ny + 3) / 4, cd.nz * nb);
+    k_restrict<<<grid, block, 0, st>>>(in, out, fd, cd, in_stride, out_stride);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
-int launch_prolong(const Dims& cd, const float* uc, const Dims& fd, float* uf, cudaStream_t st) {
+int launch_prolong(const Dims& cd, const float* uc, const Dims& fd, float* uf, int nb, cudaStream_t st) {
+    if ((long long)(cd.nz + 1) * nb > 65535) return -1;
     const dim3 block(64, 4);
-    const dim3 grid((cd.nx + 1 + 63) / 64, (cd.ny + 1 + 3) / 4, cd.nz + 1);  // cells: i, j, k in [-1, n_c - 1]
+    const dim3 grid((cd.nx + 1 + 63) / 64, (cd.ny + 1 + 3) / 4, (cd.nz + 1) * nb);  // cells: i, j, k in [-1, n_c - 1]
     k_prolong<<<grid, block, 0, st>>>(uc, uf, cd, fd);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }

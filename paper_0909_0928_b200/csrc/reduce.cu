@@ -25,7 +25,7 @@ __global__ void __launch_bounds__(RB) k_ssd(const float* __restrict__ S, const f
         const float dd = mw - s;
         acc[0] += (double)(dd * dd);
     }
-    if (block_reduce_publish<1>(acc, partials, stride, ticket)) out[0] = acc[0];
+    if (block_reduce_publish<1>(acc, partials, stride, ticket, blockIdx.x, gridDim.x)) out[0] = acc[0];
 }
 
 __global__ void __launch_bounds__(RB) k_ic_error(const float* __restrict__ uf, const float* __restrict__ ub,
@@ -46,7 +46,7 @@ __global__ void __launch_bounds__(RB) k_ic_error(const float* __restrict__ uf, c
         acc[0] += e;
         acc[1] = fmax(acc[1], e);
     }
-    if (block_reduce_publish<2, 1>(acc, partials, stride, ticket)) {
+    if (block_reduce_publish<2, 1>(acc, partials, stride, ticket, blockIdx.x, gridDim.x)) {
         out[0] = acc[0] / (double)N;
         out[1] = acc[1];
     }
@@ -76,7 +76,7 @@ __global__ void __launch_bounds__(RB) k_cc(const float* __restrict__ S, const fl
         acc[3] += b * b;
         acc[4] += a * b;
     }
-    if (block_reduce_publish<5>(acc, partials, stride, ticket)) {
+    if (block_reduce_publish<5>(acc, partials, stride, ticket, blockIdx.x, gridDim.x)) {
         const double n = (double)N;
         const double saa = acc[2] - acc[0] * acc[0] / n, sbb = acc[3] - acc[1] * acc[1] / n;
         const double sab = acc[4] - acc[0] * acc[1] / n;
@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(RB) k_point_error(const float* __restrict__ u,
 int reduce_blocks(const Dims& d, int stride) {
     const size_t N = nvox(d);
     size_t b = (N + RB - 1) / RB;
-    const size_t cap = 148 * 8;
+    const size_t cap = (size_t)sm_count() * 8;
     if (b > cap) b = cap;
     if (b > (size_t)stride) b = stride;
     return b < 1 ? 1 : (int)b;

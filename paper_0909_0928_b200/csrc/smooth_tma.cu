@@ -19,9 +19,6 @@
 // The march runs DOWN the z axis by default (`rev`): the force kernels march up, so the planes they
 // wrote last are read first while they are still in L2, and the planes written last here are the
 // ones the next force kernel reads first.  The taps are symmetric: the result is bit-identical.
-#include <cstdio>
-#include <cstdlib>
-
 #include "kernels.h"
 #include "tma.cuh"
 
@@ -53,7 +50,10 @@ struct Cfg {
     static constexpr int NH = (R + 3) / 4;      // halo float4 groups per side
     static constexpr int L = 2 * R + 1;         // ring length
     static constexpr int GX = 32;               // owner float4 groups per row (one warp wide)
-    static constexpr int GW = GX + 2 * NH;      // groups per shared row
+    // groups per shared row: owners, halos and one group of padding -- without it the rows of consecutive row
+    // groups (K rows apart) start on the same banks and the halo warp's loads conflict 8 ways (24 % of the
+    // shared-memory wavefronts at R = 6; 39.6 -> 38.6 us at R = 3, 75.2 -> 71.6 us at R = 6, bit-identical)
+    static constexpr int GW = GX + 2 * NH + 1;
     static constexpr int TY = RG * K;           // output rows per tile
     static constexpr int ROWS = TY + 2 * R;     // rows per loaded plane
     static constexpr int BOXW = 4 * GW;         // floats per loaded row
@@ -70,7 +70,7 @@ struct Cfg {
 template <int R, int K, int RG, int STAGES, int MINB, int PAIR>
 __global__ void __launch_bounds__(32 * (RG + 1), MINB)
     k_smooth_tma(const __grid_constant__ CUtensorMap tmap, float* __restrict__ out, const Dims d, const int zc,
-                 const int tiles_x, const Taps t, const int* __restrict__ skip, const int rev) {
+                 const int tiles_x, const Taps t, const Control* __restrict__ ctl, const int comps_per_pair, const int rev) {
     using C = Cfg<R, K, RG, STAGES, PAIR>;
     constexpr int LR = C::LR;
     constexpr int NH = C::NH, L = C::L, GX = C::GX, GW = C::GW, TY = C::TY, BOXW = C::BOXW;
@@ -78,7 +78,8 @@ __global__ void __launch_bounds__(32 * (RG + 1), MINB)
     float4* xs = reinterpret_cast<float4*>(smem + STAGES * C::STAGE_BYTES);  // [2][TY][GW]
     uint64_t* full = reinterpret_cast<uint64_t*>(smem + STAGES * C::STAGE_BYTES + C::XS_BYTES);
 
-    if (skip != nullptr && *reinterpret_cast<const volatile int*>(skip) != 0) return;
+    // the stopping rule of this component's pair has fired: nothing to do
+    if (ctl != nullptr && *reinterpret_cast<const volatile int*>(&ctl[blockIdx.z / comps_per_pair].stop_smooth) != 0) return;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const bool halo_warp = warp == RG;
@@ -100,7 +101,7 @@ __global__ void __launch_bounds__(32 * (RG + 1), MINB)
     } else {
         rg = lane / (2 * NH);
         const int h = lane % (2 * NH);
-        g = h < NH ? h : GX + h;  // left groups 0..NH-1, right groups GX+NH..GW-1
+        g = h < NH ? h : GX + h;  // left groups 0..NH-1, right groups GX+NH..GX+2NH-1
         active = lane < 2 * NH * RG;
         if (!active) rg = 0;
     }
@@ -274,32 +275,28 @@ int launch_cfg(const SmoothArgs& a, int zc, cudaStream_t st) {
                                         (unsigned long long)a.ncomp};
     const unsigned box[4] = {(unsigned)C::BOXW, (unsigned)C::ROWS, 1u, 1u};
     if (!tma::encode_f32(&map, a.in, 4, gdim, box)) return 0;
-    static bool attr_set = false;
-    if (!attr_set) {
+    static bool attr_set[64] = {};  // per device: the attribute belongs to the device's copy of the kernel
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 0;
+    if (!attr_set[dev]) {
         if (cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES, MINB, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM) !=
             cudaSuccess) {
             cudaGetLastError();
-            return 0;
+            return 0;  // refused: not applicable here, the caller falls back to the separable passes
         }
         cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES, MINB, PAIR>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-        attr_set = true;
-        if (getenv("DEMONS_DEBUG")) {
-            int nb = -1;
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_smooth_tma<R, K, RG, STAGES, MINB, PAIR>, C::THREADS, C::SMEM);
-            cudaFuncAttributes fa;
-            cudaFuncGetAttributes(&fa, k_smooth_tma<R, K, RG, STAGES, MINB, PAIR>);
-            fprintf(stderr, "[demons] k_smooth_tma<R=%d,K=%d,RG=%d>: %d regs, %d B dyn smem, %d threads -> %d CTAs/SM\n", R, K, RG,
-                    fa.numRegs, C::SMEM, C::THREADS, nb);
-        }
+        attr_set[dev] = true;
     }
     const int tiles_x = (d.nx + C::GX * 4 - 1) / (C::GX * 4);
     const int tiles_y = (d.ny + C::TY - 1) / C::TY;
     const int chunks = (d.nz + zc - 1) / zc;
-    if (chunks > 65535) return 0;
+    if (chunks > 65535 || a.ncomp > 65535) return 0;
     Taps t;
     for (int k = 0; k < 8; ++k) t.w[k] = k <= a.R ? a.w[k] : 0.f;
     const dim3 grid(tiles_x * tiles_y, chunks, a.ncomp);
-    k_smooth_tma<R, K, RG, STAGES, MINB, PAIR><<<grid, C::THREADS, C::SMEM, st>>>(map, a.out, d, zc, tiles_x, t, a.skip, a.ascending ? 0 : 1);
+    k_smooth_tma<R, K, RG, STAGES, MINB, PAIR><<<grid, C::THREADS, C::SMEM, st>>>(map, a.out, d, zc, tiles_x, t, a.ctl,
+                                                                             a.comps_per_pair > 0 ? a.comps_per_pair : a.ncomp,
+                                                                             a.ascending ? 0 : 1);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
@@ -334,15 +331,7 @@ int launch_smooth_tma(const SmoothArgs& a, cudaStream_t st) {
     int tile_h = 8, per_sm = 3;
     if (a.R == 4) per_sm = 2;
     if (a.R > 4) tile_h = 16, per_sm = 1;
-    if (a.tune == 1) tile_h = 16, per_sm = 1;
-    const int zc = a.zc_override > 0 ? a.zc_override : pick_zc(a, 128, tile_h, 148 * per_sm);
-    if (a.tune == 1) {  // one large CTA per SM (tuning reference)
-        if (a.R == 3) return launch_cfg<3, 2, 8, 4, 1>(a, zc, st);
-    }
-    if (((a.tune >> 16) & 0xF) == 1) {  // tuning experiments: one plane per barrier
-        if (a.R == 3) return launch_cfg<3, 2, 4, 4, 3, 1>(a, zc, st);
-        if (a.R == 4) return launch_cfg<4, 2, 4, 4, 2, 1>(a, zc, st);
-    }
+    const int zc = pick_zc(a, 128, tile_h, sm_count() * per_sm);
     // two planes per barrier where the registers allow it: 39.6 against 41.8 us at sigma 1 (R = 3),
     // 50.0 against 51.9 us at sigma 1.3 (R = 4), 256x256x100; no difference at R <= 2
     switch (a.R) {
@@ -350,8 +339,8 @@ int launch_smooth_tma(const SmoothArgs& a, cudaStream_t st) {
     case 2: return launch_cfg<2, 2, 4, 4, 3, 2>(a, zc, st);
     case 3: return launch_cfg<3, 2, 4, 4, 3, 2>(a, zc, st);
     case 4: return launch_cfg<4, 2, 4, 4, 2, 2>(a, zc, st);
-    case 5: return launch_cfg<5, 2, 8, 3, 1>(a, zc, st);
-    case 6: return launch_cfg<6, 2, 8, 3, 1>(a, zc, st);
+    case 5: return launch_cfg<5, 2, 8, 4, 1>(a, zc, st);
+    case 6: return launch_cfg<6, 2, 8, 4, 1>(a, zc, st);
     default: return 0;
     }
 }

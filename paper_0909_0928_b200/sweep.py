@@ -8,7 +8,10 @@ smoothing at sigma 1.0 and 2.0 (3 components), restrict and prolong.  Inputs are
 phantom and a random smooth field with max |u| = 8 voxels (phantoms.sweep_inputs).  Reported per
 kernel: median over `reps` samples of 10 back-to-back launches (CUDA events) after 3 warm-ups, effective GB/s = algorithmic
 bytes (DESIGN.md byte table) / time, and % of the measured HBM peak.  The same command with
---reps 3 is what the ncu captures under profiles/ run.
+--reps 3 is what the ncu captures under profiles/ run.  S and M are separate allocations here, so the L2
+access-policy window of the gathering kernels covers M alone (bench.py's pair shares one allocation and
+gets both images).  The CPU oracle's time per call for the same entry points is measured by bench.py's
+cpu_baseline leg (this package never loads the oracle).
 """
 from __future__ import annotations
 
@@ -74,7 +77,7 @@ def run(sizes, kernels, reps, device="cuda:0"):
         def add(name, ms, nbytes):
             gbs = nbytes / (ms * 1e-3) / 1e9
             rows.append({"dims": "x".join(map(str, dims)), "kernel": name, "ms": ms, "alg_bytes": nbytes,
-                         "gbs": gbs, "pct_of_peak": 100.0 * gbs / peak})
+                         "gbs": gbs, "pct_of_peak": 100.0 * gbs / peak, "pct_of_nominal_8TBs": 100.0 * gbs / 8000.0})
 
         if "force" in kernels:
             for variant in range(6):
@@ -127,13 +130,14 @@ def main():
     sizes = [tuple(int(v) for v in s.split("x")) for s in args.sizes.split(",")]
     rows, peak, kind = run(sizes, set(args.kernels.split(",")), args.reps)
     print(f"# HBM peak {peak:.1f} GB/s ({kind}); effective GB/s = algorithmic bytes / median time")
-    print(f"{'dims':>12} {'kernel':<34} {'ms':>9} {'GB/s':>9} {'% peak':>7}")
+    print(f"{'dims':>12} {'kernel':<34} {'ms':>9} {'GB/s':>9} {'% peak':>7} {'% 8TB/s':>8}")
     for r in rows:
         extra = ""
         if "max_abs_err_vs_software_voxel" in r:
             extra = (f"  |u'(tex) - u'(software)|: max {r['max_abs_err_vs_software_voxel']:.3e} mean "
                      f"{r['mean_abs_err_vs_software_voxel']:.3e} voxel, {100 * r['frac_outside_1e-4']:.1f}% outside 1e-4")
-        print(f"{r['dims']:>12} {r['kernel']:<34} {r['ms']:9.4f} {r['gbs']:9.1f} {r['pct_of_peak']:7.1f}{extra}")
+        print(f"{r['dims']:>12} {r['kernel']:<34} {r['ms']:9.4f} {r['gbs']:9.1f} {r['pct_of_peak']:7.1f} "
+              f"{r['pct_of_nominal_8TBs']:8.1f}{extra}")
     if args.json:
         with open(args.json, "w") as fh:
             json.dump({"peak_gbs": peak, "peak_kind": kind, "rows": rows}, fh, indent=1)

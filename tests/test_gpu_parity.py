@@ -326,6 +326,113 @@ def test_alpha_one_equals_double_force_on_gpu(torch_cuda, B, P):  # P8 through t
     assert np.array_equal(a["u"], b["u"])
 
 
+def run_register_batch(torch, B, variant, pairs, iters, alpha=1.0, eps=0.0, options=()):
+    """demons_register_batch on a list of (S, M) pairs of one size; returns per-pair results."""
+    nb = len(pairs)
+    S0 = pairs[0][0]
+    dims = (S0.shape[2], S0.shape[1], S0.shape[0])
+    ic = variant == 5
+    eng = B.Demons(dims, variant=variant, alpha=alpha, levels=len(iters), nbatch=nb)
+    for name, value in options:
+        B.demons_set_option(eng.ctx, name, value)
+    dS = dev(torch, np.stack([p[0] for p in pairs]))
+    dM = dev(torch, np.stack([p[1] for p in pairs]))
+    du = torch.full((nb, 3) + S0.shape, 3.0, dtype=torch.float32, device="cuda:0")   # ignored on input (multi-level)
+    dub = torch.full_like(du, -7.0) if ic else None
+    stats = np.zeros((nb, int(sum(iters)), 3))
+    done = np.zeros((nb, len(iters)), dtype=np.int32)
+    st = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    B.demons_register_batch(eng.ctx, nb, dS, dM, du, dub, iters, eps, stats, done, st)
+    torch.cuda.synchronize()
+    launches = B.demons_launch_count(eng.ctx)
+    eng.close()
+    return du.cpu().numpy(), dub.cpu().numpy() if ic else None, stats, done, launches
+
+
+@pytest.mark.parametrize("variant", [0, 1, 3, 5])
+def test_register_batch_equals_single_calls(torch_cuda, B, P, variant):
+    """demons_register_batch: every pair of the batch gets the field demons_register gives it alone, bit for
+    bit; the statistics agree to rounding (the block partition of the reduction differs with the batch)."""
+    dims = (44, 36, 22)
+    iters = [9, 7, 6]
+    pairs = [P.config1_pair(dims=dims, seed=300 + k, max_norm=1.5 + 0.3 * k)[:2] for k in range(5)]
+    u, ub, stats, done, launches = run_register_batch(torch_cuda, B, variant, pairs, iters, alpha=ALPHA.get(variant, 1.0))
+    singles = 0
+    for k, (S, M) in enumerate(pairs):
+        one = run_register(torch_cuda, B, variant, S, M, iters, alpha=ALPHA.get(variant, 1.0))
+        singles += one["launches"]
+        assert np.array_equal(u[k], one["u"]), f"pair {k}"
+        if variant == 5:
+            assert np.array_equal(ub[k], one["ub"])
+        np.testing.assert_allclose(stats[k], one["stats"], rtol=1e-12, atol=0)
+        assert done[k].tolist() == one["iters_done"]
+    assert launches <= 1.1 * singles / len(pairs)    # every level small enough to run as ONE group: a single registration's launch count
+
+
+def test_register_batch_groups_and_early_stop(torch_cuda, B, P, oracle):
+    """Levels large enough to fill the GPU run in groups of pairs (here 3 + 1 on the finest level), and with
+    eps > 0 every pair stops on its own iteration, as its single registration does."""
+    torch = torch_cuda
+    dims = (160, 128, 64)   # 1.3 Mvoxel: groups of 3 pairs on the finest level, the whole batch below it
+    pairs = [P.config1_pair(dims=dims, seed=400 + k, noise_sd=0.0, max_norm=1.0 + 0.5 * k)[:2] for k in range(4)]
+    iters = [14, 12]
+    u, _, stats, done, _ = run_register_batch(torch, B, 0, pairs, iters)
+    for k, (S, M) in enumerate(pairs):
+        one = run_register(torch, B, 0, S, M, iters)
+        assert np.array_equal(u[k], one["u"]), f"pair {k}"
+    # early stop, small volumes: different pairs stop at different iterations
+    dims = (32, 32, 16)
+    pairs = [P.config1_pair(dims=dims, seed=9 + k, noise_sd=0.0, max_norm=1.0 + 0.4 * k)[:2] for k in range(4)]
+    eps = 3e-3
+    u, _, stats, done, _ = run_register_batch(torch, B, 0, pairs, [60], eps=eps, options=(("zero_start", 1),))
+    stops = []
+    for k, (S, M) in enumerate(pairs):
+        one = run_register(torch, B, 0, S, M, [60], eps=eps)
+        assert np.array_equal(u[k], one["u"]), f"pair {k}"
+        assert done[k].tolist() == one["iters_done"]
+        n = one["iters_done"][0]
+        assert np.all(stats[k, n:] == 0.0)
+        stops.append(n)
+    assert len(set(stops)) > 1 and min(stops) < 60, stops
+
+
+def test_inverse_consistent_one_field_is_bit_identical(torch_cuda, B, P, oracle):
+    """Variant 5 from a zero start iterates on u_f alone (u_b = -u_f, pin P10) and writes u_b on exit: same
+    bits, fields and statistics, as iterating on both fields ("ic_one_field" = 0)."""
+    torch = torch_cuda
+    dims = (44, 36, 22)
+    S, M, _ = P.config1_pair(dims=dims, seed=77, max_norm=2.5)
+    res = {}
+    for one_field in (1, 0):
+        eng = B.Demons(dims, variant=5, levels=3)
+        B.demons_set_option(eng.ctx, "ic_one_field", one_field)
+        du = torch.zeros((3,) + S.shape, dtype=torch.float32, device="cuda:0")
+        dub = torch.zeros_like(du)
+        stats = np.zeros((30, 3))
+        st = torch.cuda.Stream()
+        torch.cuda.synchronize()
+        B.demons_register(eng.ctx, dev(torch, S), dev(torch, M), du, dub, [12, 10, 8], 0.0, stats, None, st)
+        torch.cuda.synchronize()
+        res[one_field] = (du.cpu().numpy(), dub.cpu().numpy(), stats, B.demons_launch_count(eng.ctx))
+        eng.close()
+    assert np.array_equal(res[1][0], res[0][0]) and np.array_equal(res[1][1], res[0][1])
+    assert np.array_equal(res[1][1], -res[1][0])
+    assert np.array_equal(res[1][2], res[0][2])
+    assert res[1][3] < res[0][3]      # one smoothing launch per iteration instead of two
+    # a caller-supplied pair of fields (single level, no zero start) keeps the two-field form
+    u0 = P.bump_field(dims, np.random.default_rng(5), 4, (3.0, 8.0), 1.0, centre_frac=1.0)
+    ub0 = P.bump_field(dims, np.random.default_rng(6), 4, (3.0, 8.0), 1.0, centre_frac=1.0)
+    eng = B.Demons(dims, variant=5, levels=1)
+    du, dub = dev(torch, u0), dev(torch, ub0)
+    B.demons_register(eng.ctx, dev(torch, S), dev(torch, M), du, dub, [3])
+    torch.cuda.synchronize()
+    assert not np.array_equal(dub.cpu().numpy(), -du.cpu().numpy())
+    ref = oracle.register(5, 1.0, 1.0, S, M, [3], u0=u0, ub0=ub0)
+    assert np.abs(du.cpu().numpy() - ref["u"]).max() <= 1e-3 and np.abs(dub.cpu().numpy() - ref["ub"]).max() <= 1e-3
+    eng.close()
+
+
 def test_api_rejects_bad_calls(torch_cuda, B):
     torch = torch_cuda
     dims = (16, 16, 8)
@@ -363,12 +470,16 @@ def lung_case(P):
     return S, M, u
 
 
-def force_atol(oracle, variant, S, M, u, ub):
+FORCE_BOUND = {0: 0.5, 1: 0.54433, 2: 0.5, 3: 1.0, 5: 0.5}   # P9; variant 4: 1/alpha
+
+
+def force_atol(oracle, variant, S, M, u, ub, alpha=1.0):
     """Per-voxel absolute tolerance of u_out at HU-scale intensities (tolerance derivation).
     Eq.(1)-(6) are d g / (d^2 + |g|^2) terms: |dF/dd| reaches 1/|g| at d = 0, and d = Mw - S carries
     the fp32 rounding of the trilinear sample, up to 2 ulp(|I|max) against the oracle's fp64 lerp.
     Where the gradient is below ~1 HU/voxel that alone exceeds 1e-4, so the bound is
-    1e-4 + 4 ulp * (sum over the force terms of 1/|g|), capped at 1 (|F| <= 1)."""
+    1e-4 + 4 ulp * (sum over the force terms of 1/|g|), capped at the variant's own bound on |F| (SURVEY.md
+    pin P9: 1/2 for Eq.1, 3, 6; 0.54433 for Eq.2; 1 for Eq.4; 1/alpha for Eq.5)."""
     def norm(g):
         return np.sqrt((g.astype(np.float64) ** 2).sum(axis=0))
     ulp = float(np.spacing(np.float32(max(np.abs(S).max(), np.abs(M).max()))))
@@ -387,18 +498,20 @@ def force_atol(oracle, variant, S, M, u, ub):
             sens = 2.0 / np.maximum(norm(oracle.gradient(Mw)), tiny)
             if variant in (3, 4):
                 sens = sens + 1.0 / np.maximum(gS, tiny)
-    return np.minimum(1e-4 + 4.0 * ulp * sens, 1.0)[None]
+    cap = 1.0 / alpha if variant == 4 else FORCE_BOUND[variant]
+    return np.minimum(1e-4 + 4.0 * ulp * sens, cap)[None]
 
 
-@pytest.mark.parametrize("variant", [0, 1, 3, 5])
+@pytest.mark.parametrize("variant", VARIANTS)
 def test_full_size_warp_force_matches_oracle(torch_cuda, B, oracle, lung_case, variant):
     """Every voxel of the 256x256x100 pass (the oracle takes about a second per call)."""
     torch = torch_cuda
     S, M, u = lung_case
     ic = variant == 5
     ub = (-u).copy()
-    ref_u, ref_ub, ref_m = oracle.warp_force(variant, 1.0, S, M, u, ub if ic else None)
-    eng = B.Demons(FULL_DIMS, variant=variant)
+    alpha = ALPHA.get(variant, 1.0)
+    ref_u, ref_ub, ref_m = oracle.warp_force(variant, alpha, S, M, u, ub if ic else None)
+    eng = B.Demons(FULL_DIMS, variant=variant, alpha=alpha)
     du = dev(torch, u)
     out = torch.full_like(du, float("nan"))
     outb = torch.full_like(du, float("nan")) if ic else None
@@ -406,9 +519,13 @@ def test_full_size_warp_force_matches_oracle(torch_cuda, B, oracle, lung_case, v
     B.demons_warp_force(eng.ctx, FULL_DIMS, dev(torch, S), dev(torch, M), du, out, dev(torch, ub) if ic else None,
                         outb, met)
     torch.cuda.synchronize()
-    atol = force_atol(oracle, variant, S, M, u, ub)
+    atol = force_atol(oracle, variant, S, M, u, ub, alpha)
     assert float((atol > 1e-3).mean()) < 1e-3  # the conditioning term matters for a handful of voxels only
-    assert_close(out.cpu().numpy(), ref_u, f"full-size u_out variant {variant}", atol=atol)
+    got = out.cpu().numpy()
+    plain = np.abs(got.astype(np.float64) - ref_u) > 1e-4 + 1e-5 * np.abs(ref_u)
+    print(f"\nvariant {variant}: {int(plain.sum())} of {plain.size} elements outside the plain 1e-4 + 1e-5|ref| bar "
+          f"(all inside the conditioned bound); the bound exceeds 1e-3 at {int((atol > 1e-3).sum())} voxels")
+    assert_close(got, ref_u, f"full-size u_out variant {variant}", atol=atol)
     if ic:
         assert_close(outb.cpu().numpy(), ref_ub, "full-size ub_out", atol=atol)
     np.testing.assert_allclose(met.cpu().numpy(), ref_m, rtol=1e-5)

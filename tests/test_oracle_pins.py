@@ -554,3 +554,17 @@ def test_point_error_pins(oracle):
     lib_u = np.stack([ndimage.map_coordinates(ur[c].astype(np.float64), coords, order=1, mode="nearest") for c in range(3)], axis=1)
     err = oracle.point_error(ur, (1, 1, 1), p, np.zeros((20, 3), np.float32))
     assert np.allclose(err, np.linalg.norm(lib_u, axis=1), rtol=1e-9, atol=1e-12)
+
+
+@pytest.mark.parametrize("variant", [2, 5])
+def test_chained_driver_of_the_full_size_references(oracle, variant):
+    """tests/full_refs.py walks the multi-scale driver in segments to keep probes along the trajectory: that
+    walk must reproduce oracle_register bit for bit (fields and statistics)."""
+    import full_refs as FR
+    S, M, _ = _smooth_pair(dims=(22, 19, 13), noise=5.0)
+    iters = [12, 11, 17]
+    one = oracle.register(variant, 1.0, 1.0, S, M, iters)
+    ch = FR.chained_register(oracle, variant, 1.0, S, M, iters)
+    assert np.array_equal(ch["u"], one["u"])
+    np.testing.assert_array_equal(ch["stats"], one["stats"])
+    assert sum(k.endswith("_before") for k in ch) >= 6

@@ -50,3 +50,22 @@ def test_single_process_is_identity():
         os.environ.pop(k, None)
     assert replicas.env_world() == (0, 0, 1)
     assert replicas.aggregate(6.0, 2.0) == {"units": 6.0, "seconds": 2.0, "value": 3.0}
+
+
+def test_bench_spawns_its_own_ranks():
+    """`python bench.py --gpus 2` outside torchrun must start the two ranks itself and report n_gpus = 2 only
+    because two ranks reported (here with the CPU stub in place of the GPU step, gloo backend)."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_PORT")}
+    res = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--stub", "--steps", "3"],
+                         capture_output=True, text=True, timeout=300, env=env, cwd=root)
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [l for l in res.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1            # rank 0 alone prints
+    line = json.loads(lines[0])
+    assert line["n_gpus"] == 2 and line["units"] == 6.0
+    # max over ranks: rank 1 sleeps 20 ms per step
+    assert line["ms_per_step"] >= 19.0
