@@ -8,7 +8,7 @@ smoothing at sigma 1.0 and 2.0 (3 components), restrict and prolong.  Inputs are
 phantom and a random smooth field with max |u| = 8 voxels (phantoms.sweep_inputs).  Reported per
 kernel: median over `reps` samples of 10 back-to-back launches (CUDA events) after 3 warm-ups, effective GB/s = algorithmic
 bytes (DESIGN.md byte table) / time, and % of the measured HBM peak.  The same command with
---reps 3 is what the ncu captures under profiles/ run.  S and M are separate allocations here, so the L2
+--reps 1 --warmups 1 --inner 1 (every entry point launched twice) is what the ncu captures under profiles/ run.  S and M are separate allocations here, so the L2
 access-policy window of the gathering kernels covers M alone (bench.py's pair shares one allocation and
 gets both images).  The CPU oracle's time per call for the same entry points is measured by bench.py's
 cpu_baseline leg (this package never loads the oracle).
@@ -39,10 +39,14 @@ def hbm_peak():
         return 6650.0, "fallback"
 
 
-def median_ms(torch, stream, fn, reps, inner=10):
+WARMUPS, INNER = 3, 10
+
+
+def median_ms(torch, stream, fn, reps, inner=None):
     """Median over `reps` samples of (CUDA-event time of `inner` back-to-back launches) / inner: the
     queue stays full, so the host's launch latency is not in the number."""
-    for _ in range(3):
+    inner = INNER if inner is None else inner
+    for _ in range(WARMUPS):
         fn()
     torch.cuda.synchronize()
     times = []
@@ -126,7 +130,11 @@ def main():
     ap.add_argument("--kernels", default="force,smooth,pyramid,texture")
     ap.add_argument("--reps", type=int, default=20)
     ap.add_argument("--json", default=None)
+    ap.add_argument("--warmups", type=int, default=3)
+    ap.add_argument("--inner", type=int, default=10, help="back-to-back launches per timed sample")
     args = ap.parse_args()
+    global WARMUPS, INNER
+    WARMUPS, INNER = args.warmups, args.inner
     sizes = [tuple(int(v) for v in s.split("x")) for s in args.sizes.split(",")]
     rows, peak, kind = run(sizes, set(args.kernels.split(",")), args.reps)
     print(f"# HBM peak {peak:.1f} GB/s ({kind}); effective GB/s = algorithmic bytes / median time")
