@@ -170,6 +170,22 @@ int demons_warp_force(demons_ctx* ctx, const int dims[3], const float* d_static,
                       const float* d_moving, const float* d_u_in, float* d_u_out,
                       const float* d_ub_in, float* d_ub_out, double* d_metrics, void* stream);
 
+/* demons_warp_force_slab: the same pass for ONE RANK of a z-slab decomposition (volumes of
+ * 512x512x256 and up, one slab of planes per GPU).  dims = the WHOLE volume; d_static and d_moving are whole
+ * volumes (replicated on every rank, so that the gather of PAPER.md L179 never leaves the device); the fields are
+ * the rank's slab only: planes [z_begin, z_begin + z_count) of the volume, [3][z_count*ny*nx], own planes plus
+ * halo planes.  Every image access uses global planes and the clamps of the whole volume; gradients of the warped
+ * images (variants 2-5) are taken inside the slab, so the OUTERMOST plane of a slab side that is not a face of the
+ * volume comes out wrong and must be halo.  With R = ceil(3 sigma), a halo of R + 1 planes per interior side makes
+ * [warp_force_slab ; demons_smooth on the slab] exact on the own planes; the caller then refreshes the halos from
+ * the neighbours' own planes (paper_0909_0928_b200/slabs.py: torch.distributed send/recv, one exchange per
+ * iteration).  d_metrics (nullable): the three sums over planes [own_begin, own_begin + own_count) of the SLAB
+ * (local indices), to be added over the ranks.  The context must have been created with the whole volume's dims;
+ * z_count >= 2.  The "texture" option is not served. */
+int demons_warp_force_slab(demons_ctx* ctx, const int dims[3], int z_begin, int z_count, int own_begin, int own_count,
+                           const float* d_static, const float* d_moving, const float* d_u_in, float* d_u_out,
+                           const float* d_ub_in, float* d_ub_out, double* d_metrics, void* stream);
+
 /* demons_smooth: S5 -- separable Gaussian of `ncomp` planar components, radius R = ceil(3 sigma),
  * normalised taps, clamped borders (reading A9).  d_in != d_out. */
 int demons_smooth(demons_ctx* ctx, const int dims[3], const float* d_in, float* d_out, int ncomp,

@@ -40,6 +40,8 @@ SIGNATURES = {
     "demons_register_host": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, ctypes.c_int, _c_int3, ctypes.c_double, _vp,
                                             _vp, _vp]),
     "demons_warp_force": (ctypes.c_int, [_vp, _c_int3, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "demons_warp_force_slab": (ctypes.c_int, [_vp, _c_int3, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp,
+                                              _vp, _vp, _vp, _vp, _vp, _vp]),
     "demons_smooth": (ctypes.c_int, [_vp, _c_int3, _vp, _vp, ctypes.c_int, ctypes.c_float, _vp]),
     "demons_restrict": (ctypes.c_int, [_vp, _c_int3, _vp, _vp, _vp]),
     "demons_prolong": (ctypes.c_int, [_vp, _c_int3, _vp, _c_int3, _vp, _vp]),
@@ -183,6 +185,13 @@ def demons_warp_force(ctx, dims, d_static, d_moving, d_u_in, d_u_out, d_ub_in=No
                       stream=None):
     _check(lib().demons_warp_force(ctx, _int3(dims), _ptr(d_static), _ptr(d_moving), _ptr(d_u_in), _ptr(d_u_out),
                                    _ptr(d_ub_in), _ptr(d_ub_out), _ptr(d_metrics), _stream(stream)))
+
+
+def demons_warp_force_slab(ctx, dims, z_begin, z_count, own_begin, own_count, d_static, d_moving, d_u_in, d_u_out,
+                           d_ub_in=None, d_ub_out=None, d_metrics=None, stream=None):
+    _check(lib().demons_warp_force_slab(ctx, _int3(dims), int(z_begin), int(z_count), int(own_begin), int(own_count),
+                                        _ptr(d_static), _ptr(d_moving), _ptr(d_u_in), _ptr(d_u_out), _ptr(d_ub_in),
+                                        _ptr(d_ub_out), _ptr(d_metrics), _stream(stream)))
 
 
 def demons_smooth(ctx, dims, d_in, d_out, ncomp, sigma, stream=None):

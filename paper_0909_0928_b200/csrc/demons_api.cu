@@ -816,6 +816,61 @@ int demons_warp_force(demons_ctx* c, const int dims[3], const float* d_static, c
     return DEMONS_OK;
 }
 
+int demons_warp_force_slab(demons_ctx* c, const int dims[3], int z_begin, int z_count, int own_begin, int own_count,
+                           const float* d_static, const float* d_moving, const float* d_u_in, float* d_u_out,
+                           const float* d_ub_in, float* d_ub_out, double* d_metrics, void* stream) {
+    if (!c) return fail(DEMONS_E_ARG, "ctx is NULL");
+    Dims g;
+    int rc = check_call_dims(c, dims, &g);
+    if (rc != DEMONS_OK) return rc;
+    if (g.nx < 2 || g.ny < 2 || g.nz < 2) return fail(DEMONS_E_UNSUPPORTED, "the slab form needs at least 2 voxels per axis");
+    if (z_begin < 0 || z_count < 2 || z_begin + z_count > g.nz) return fail(DEMONS_E_ARG, "slab outside the volume");
+    if (own_begin < 0 || own_count < 0 || own_begin + own_count > z_count) return fail(DEMONS_E_ARG, "own planes outside the slab");
+    if (!d_static || !d_moving || !d_u_in || !d_u_out) return fail(DEMONS_E_ARG, "NULL volume / field pointer");
+    if (d_u_in == d_u_out) return fail(DEMONS_E_ARG, "u_out must not alias u_in");
+    const bool ic = is_ic(c);
+    if (ic && (!d_ub_in || !d_ub_out)) return fail(DEMONS_E_ARG, "variant 5 needs ub_in and ub_out");
+    if (!ic && (d_ub_in || d_ub_out)) return fail(DEMONS_E_ARG, "ub_in / ub_out must be NULL unless variant 5");
+    if (c->opt_texture) return fail(DEMONS_E_UNSUPPORTED, "the texture option serves whole volumes only");
+    rc = check_ws(c, 1);
+    if (rc != DEMONS_OK) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const Partition p = make_partition(c, 1, 1);
+    ForceArgs fa{};
+    fa.d = Dims{g.nx, g.ny, z_count};
+    fa.variant = c->variant;
+    fa.alpha2 = c->variant == DEMONS_ADJUSTED_DOUBLE ? c->alpha * c->alpha : 1.f;
+    fa.nb = 1;
+    fa.img_stride = nvox(g);
+    fa.S = d_static;
+    fa.M = d_moving;
+    fa.u_in = d_u_in;
+    fa.u_out = d_u_out;
+    fa.ub_in = d_ub_in;
+    fa.ub_out = d_ub_out;
+    fa.Mw = reinterpret_cast<float*>(c->ws + p.Mw);  // variant 1: |grad M|^2 in GLOBAL indexing; else the slab's Mw
+    fa.Sw = ic ? reinterpret_cast<float*>(c->ws + p.Sw) : nullptr;
+    fa.sink = make_sink(c, p, 0, d_metrics, 0, false, 0.0);
+    fa.slab = 1;
+    fa.zoff = z_begin;
+    fa.gnz = g.nz;
+    fa.mz0 = own_begin;
+    fa.mz1 = own_begin + own_count;
+    const L2Window win = l2_window(c, g, d_static, d_moving, nvox(g), 1);
+    fa.l2_ptr = win.ptr;
+    fa.l2_bytes = win.bytes;
+    fa.l2_ratio = win.ratio;
+    if (c->variant == DEMONS_EVOLVED_PASSIVE) {  // the planes of this slab only
+        if (launch_grad_mag2(g, d_moving, nvox(g), fa.Mw, 1, st, z_begin, z_count) < 0)
+            return fail(DEMONS_E_CUDA, "gradient launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        c->launches += 1;
+    }
+    const int n = launch_warp_force(fa, st);
+    if (n < 0) return fail(DEMONS_E_CUDA, "warp_force launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    c->launches += n;
+    return DEMONS_OK;
+}
+
 int demons_smooth(demons_ctx* c, const int dims[3], const float* d_in, float* d_out, int ncomp, float sigma,
                   void* stream) {
     if (!c) return fail(DEMONS_E_ARG, "ctx is NULL");

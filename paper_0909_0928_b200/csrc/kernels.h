@@ -28,6 +28,10 @@ struct ForceArgs {
     MetricSink sink;
     cudaTextureObject_t texM;  // 0 = software trilinear (default); nb must be 1 otherwise
     cudaEvent_t ev_mid;        // nullable: recorded between the warp and the force kernel (profiling)
+    // z-slab form (one rank of a z-slab decomposition): d is the local slab (fields, warped images), which starts at
+    // plane zoff of the images; S and M are whole volumes of gnz planes; planes [mz0, mz1) of the slab count in the
+    // metrics.  nb must be 1, texM 0.
+    int slab, zoff, gnz, mz0, mz1;
     // L2 access-policy window of the gathering kernels (persisting); l2_bytes == 0: none
     const void* l2_ptr;
     size_t l2_bytes;
@@ -39,7 +43,9 @@ int launch_warp_force(const ForceArgs& a, cudaStream_t stream);
 
 // Variant 1, once per level (and per standalone demons_warp_force call): out <- |grad I|^2, [nb][N], which
 // launch_warp_force then reads instead of stencilling M (Eq.(2) uses only the magnitude of grad M0).
-int launch_grad_mag2(const Dims& d, const float* I, size_t img_stride, float* out, int nb, cudaStream_t stream);
+// Planes [z0, z0 + zn) of the volume only (zn < 0: all of them).
+int launch_grad_mag2(const Dims& d, const float* I, size_t img_stride, float* out, int nb, cudaStream_t stream,
+                     int z0 = 0, int zn = -1);
 
 // out[nb][3][N] = -in: the backward field of variant 5 on exit from the one-field form (u_b = -u_f, P10).
 int launch_negate(const float* in, float* out, size_t n, cudaStream_t stream);

@@ -89,6 +89,9 @@ struct KParams {
     unsigned img_stride;  // floats between the images of consecutive pairs
     int zper;             // consecutive planes per block
     int chunks;           // z chunks per pair; blockIdx.z = pair * chunks + chunk
+    // z-slab form (SLAB kernels): the fields and warped images are a slab of d.nz planes that starts at plane zoff of
+    // the images, which are whole volumes of gnz planes; only planes [mz0, mz1) of the slab count in the metrics
+    int zoff, gnz, mz0, mz1;
 };
 
 // Pair b of a batched launch: every pointer moves to that pair's data.
@@ -261,7 +264,9 @@ struct PlaneRegs {
 // boundary, 64.3 us without (the same instructions, a different order).
 // BATCH = false is the single-registration launch (blockIdx.z is the z chunk, every pointer stays a kernel
 // parameter): the pair offsets of a batch cost registers that the 128-register configuration does not have.
-template <int VARIANT, int XPT, bool FULL, bool TEX, int MINB, bool BATCH>
+// SLAB = true: one rank's share of a z-slab decomposition (see KParams): every image access (the gather from M, the
+// stencil of S, |grad M|^2) is in global planes z + zoff with the clamps of the whole volume; the field is local.
+template <int VARIANT, int XPT, bool FULL, bool TEX, int MINB, bool BATCH, bool SLAB = false>
 __global__ void __launch_bounds__(BX* BY, MINB) k_force_fixed_lc(const KParams p0) {
     const unsigned b = BATCH ? blockIdx.z / (unsigned)p0.chunks : 0u;
     const unsigned cz = BATCH ? blockIdx.z - b * (unsigned)p0.chunks : blockIdx.z;
@@ -281,6 +286,9 @@ __global__ void __launch_bounds__(BX* BY, MINB) k_force_fixed_lc(const KParams p
         const int zb = (int)cz * p.zper, ze = min(d.nz, zb + p.zper);
         const unsigned plane = (unsigned)(d.nx * d.ny);
         const unsigned row0 = (unsigned)((zb * d.ny + y) * d.nx + xb);
+        const int zoff = SLAB ? p.zoff : 0;                               // image plane of field plane 0
+        const Dims dg = SLAB ? Dims{d.nx, d.ny, p.gnz} : d;               // dims of the images
+        const unsigned rowS0 = row0 + (unsigned)zoff * plane;             // the same voxel in the images
         const unsigned dym = y > 0 ? (unsigned)d.nx : 0u, dyp = y < d.ny - 1 ? (unsigned)d.nx : 0u;
         float nux[XPT], nuy[XPT], nuz[XPT];  // field of the plane after the one being issued
         float sm[XPT], sc[XPT];  // centre values of S on planes z-1 and z
@@ -305,21 +313,22 @@ __global__ void __launch_bounds__(BX* BY, MINB) k_force_fixed_lc(const KParams p
                 q.uy[j] = nuy[j];
                 q.uz[j] = nuz[j];
             }
-            const unsigned dzp = z < d.nz - 1 ? plane : 0u;
+            const unsigned rowS = rowS0 + (unsigned)(z - zb) * plane;
+            const unsigned dzp = z + zoff < dg.nz - 1 ? plane : 0u;
             if (z + 1 < ze) load_u(row + plane);
             if (rt) {
-                load_stencil<XPT, FULL>(p.S, r, row, dym, dyp, dzp, q.ss);
+                load_stencil<XPT, FULL>(p.S, r, rowS, dym, dyp, dzp, q.ss);
                 if constexpr (VARIANT == 1) {
-                    const float* pg = p.gm2 + row;
+                    const float* pg = p.gm2 + rowS;
 #pragma unroll
                     for (int j = 0; j < XPT; ++j) q.m2[j] = (FULL || r.ok[j]) ? __ldg(pg + 32 * j) : 0.f;
                 }
             }
             if constexpr (!TEX) {
                 unsigned o[XPT];
-                make_cells<XPT>(d, xs, y, z, q.ux, q.uy, q.uz, o, q.fx, q.fy, q.fz);
+                make_cells<XPT>(dg, xs, y, z + zoff, q.ux, q.uy, q.uz, o, q.fx, q.fy, q.fz);
 #pragma unroll
-                for (int j = 0; j < XPT; ++j) load_cell(p.M, d, o[j], q.c[j]);
+                for (int j = 0; j < XPT; ++j) load_cell(p.M, dg, o[j], q.c[j]);
             }
         };
         auto finish = [&](PlaneRegs<VARIANT, XPT>& q, int z) {
@@ -328,6 +337,7 @@ __global__ void __launch_bounds__(BX* BY, MINB) k_force_fixed_lc(const KParams p
             float* o1 = p.u_out + (N + row);
             float* o2 = p.u_out + (2 * N + row);
             float ssd = 0.f, sf = 0.f, su = 0.f;
+            const bool counted = !SLAB || (z >= p.mz0 && z < p.mz1);  // halo planes of a slab belong to a neighbour
 #pragma unroll
             for (int j = 0; j < XPT; ++j) {
                 float mw;
@@ -361,14 +371,16 @@ __global__ void __launch_bounds__(BX* BY, MINB) k_force_fixed_lc(const KParams p
                     su += fast_sqrt(fmaf(q.ux[j], q.ux[j], fmaf(q.uy[j], q.uy[j], q.uz[j] * q.uz[j])));
                 }
             }
-            acc[0] += (double)ssd;
-            acc[1] += (double)sf;
-            acc[2] += (double)su;
+            if (counted) {
+                acc[0] += (double)ssd;
+                acc[1] += (double)sf;
+                acc[2] += (double)su;
+            }
         };
 
         load_u(row0);
         {
-            const float *qs = p.S + row0, *qsm = p.S + (row0 - (zb > 0 ? plane : 0u));
+            const float *qs = p.S + rowS0, *qsm = p.S + (rowS0 - (zb + zoff > 0 ? plane : 0u));
 #pragma unroll
             for (int j = 0; j < XPT; ++j) {
                 const bool ok = FULL || r.ok[j];
@@ -387,9 +399,9 @@ __global__ void __launch_bounds__(BX* BY, MINB) k_force_fixed_lc(const KParams p
 
 // |grad M|^2 of a level image (central differences, clamped; O1), once per level for variant 1.
 __global__ void __launch_bounds__(256) k_grad_mag2(const float* __restrict__ I, float* __restrict__ out, const Dims d,
-                                                   const size_t img_stride) {
+                                                   const size_t img_stride, const int z0, const int zn) {
     const int x = blockIdx.x * 64 + threadIdx.x, y = blockIdx.y * 4 + threadIdx.y;
-    const int b = blockIdx.z / d.nz, z = blockIdx.z - b * d.nz;  // blockIdx.z = pair * nz + z
+    const int b = blockIdx.z / zn, z = z0 + (int)(blockIdx.z - b * zn);  // blockIdx.z = pair * zn + (z - z0)
     if (x >= d.nx || y >= d.ny) return;
     I += (size_t)b * img_stride;
     out += (size_t)b * nvox(d);
@@ -400,11 +412,48 @@ __global__ void __launch_bounds__(256) k_grad_mag2(const float* __restrict__ I, 
     out[i] = fmaf(gx, gx, fmaf(gy, gy, gz * gz));
 }
 
+// The same for rows that are a whole number of float4s: a thread owns one float4 of a row and marches along z with
+// the planes z-1, z, z+1 rolling through registers (one 128-bit load of new data per plane; the y neighbours and the
+// two x edge values come from L1).  Same arithmetic per voxel as k_grad_mag2.
+__global__ void __launch_bounds__(256) k_grad_mag2_v4(const float* __restrict__ I, float* __restrict__ out, const Dims d,
+                                                      const size_t img_stride, const int zper, const int chunks,
+                                                      const int z0, const int zn) {
+    const int x0 = 4 * (blockIdx.x * 32 + threadIdx.x), y = blockIdx.y * 8 + threadIdx.y;
+    const int b = blockIdx.z / chunks, cz = blockIdx.z - b * chunks;
+    if (x0 >= d.nx || y >= d.ny) return;
+    I += (size_t)b * img_stride;
+    out += (size_t)b * nvox(d);
+    const unsigned plane = (unsigned)(d.nx * d.ny);
+    const int zb = z0 + cz * zper, ze = min(z0 + zn, zb + zper);  // planes [z0, z0 + zn) of the volume
+    unsigned i = (unsigned)((zb * d.ny + y) * d.nx + x0);
+    const unsigned dym = y > 0 ? (unsigned)d.nx : 0u, dyp = y < d.ny - 1 ? (unsigned)d.nx : 0u;
+    const unsigned dxm = x0 > 0 ? 1u : 0u, dxp = x0 + 4 < d.nx ? 4u : 3u;
+    float4 lo = __ldg(reinterpret_cast<const float4*>(I + i - (zb > 0 ? plane : 0u)));
+    float4 c = __ldg(reinterpret_cast<const float4*>(I + i));
+    for (int z = zb; z < ze; ++z, i += plane) {
+        const float4 hi = __ldg(reinterpret_cast<const float4*>(I + i + (z < d.nz - 1 ? plane : 0u)));
+        const float4 ym = __ldg(reinterpret_cast<const float4*>(I + i - dym)), yp = __ldg(reinterpret_cast<const float4*>(I + i + dyp));
+        const float xl = __ldg(I + i - dxm), xr = __ldg(I + i + dxp);
+        const float cv[6] = {xl, c.x, c.y, c.z, c.w, xr};
+        const float ymv[4] = {ym.x, ym.y, ym.z, ym.w}, ypv[4] = {yp.x, yp.y, yp.z, yp.w};
+        const float lov[4] = {lo.x, lo.y, lo.z, lo.w}, hiv[4] = {hi.x, hi.y, hi.z, hi.w};
+        float o[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const float gx = 0.5f * (cv[e + 2] - cv[e]), gy = 0.5f * (ypv[e] - ymv[e]), gz = 0.5f * (hiv[e] - lov[e]);
+            o[e] = fmaf(gx, gx, fmaf(gy, gy, gz * gz));
+        }
+        *reinterpret_cast<float4*>(out + i) = make_float4(o[0], o[1], o[2], o[3]);
+        lo = c;
+        c = hi;
+    }
+}
+
 // Pass 1 of variants 2-5 in the same layout: Mw = warp(M, u)  (variant 5 also Sw = warp(S, ub)).
 // IC: 0 = variants 2-4; 1 = variant 5 with two stored fields; 2 = variant 5 in the one-field form, where
 // u_b = -u_f exactly (pin P10: from a zero start negation commutes with every operation of the iteration),
 // so S is warped by the negated registers of u and the second field is never read.
-template <int XPT, bool FULL, int IC, bool TEX>
+template <int XPT, bool FULL, int IC, bool TEX, bool SLAB = false>
 __global__ void __launch_bounds__(BX* BY) k_warp_lc(const KParams p0) {
     const unsigned b = blockIdx.z / (unsigned)p0.chunks, cz = blockIdx.z - b * (unsigned)p0.chunks;
     if (skip_pass(p0.sink, b)) return;
@@ -422,6 +471,8 @@ __global__ void __launch_bounds__(BX* BY) k_warp_lc(const KParams p0) {
     const int zb = (int)cz * p.zper, ze = min(d.nz, zb + p.zper);
     const unsigned plane = (unsigned)(d.nx * d.ny);
     unsigned row = (unsigned)((zb * d.ny + y) * d.nx + xb);
+    const int zoff = SLAB ? p.zoff : 0;                  // image plane of field plane 0 (z-slab form)
+    const Dims dg = SLAB ? Dims{d.nx, d.ny, p.gnz} : d;  // dims of the images
     constexpr int NF = IC == 1 ? 2 : 1;  // fields loaded: u (warps M), u_b (warps S)
     constexpr int NW = IC != 0 ? 2 : 1;  // images warped
     float nux[NF][XPT], nuy[NF][XPT], nuz[NF][XPT];  // the field(s) of the next plane (register prefetch)
@@ -464,9 +515,9 @@ __global__ void __launch_bounds__(BX* BY) k_warp_lc(const KParams p0) {
             } else {
                 unsigned o[XPT];
                 float fx[XPT], fy[XPT], fz[XPT], c[XPT][8];
-                make_cells<XPT>(d, xs, y, z, ux[f], uy[f], uz[f], o, fx, fy, fz);
+                make_cells<XPT>(dg, xs, y, z + zoff, ux[f], uy[f], uz[f], o, fx, fy, fz);
 #pragma unroll
-                for (int j = 0; j < XPT; ++j) load_cell(I, d, o[j], c[j]);
+                for (int j = 0; j < XPT; ++j) load_cell(I, dg, o[j], c[j]);
 #pragma unroll
                 for (int j = 0; j < XPT; ++j) v[j] = lerp_cell(c[j], fx[j], fy[j], fz[j]);
             }
@@ -501,7 +552,9 @@ __global__ void __launch_bounds__(BX* BY) k_warp(const KParams p0) {
 
 // ---- variants 2-5, pass 2: gradient of the warped image(s), force, update ---------------------
 // ONEF (variant 5 only): the one-field form -- u_b' = u_b + F = -(u - F) = -u' exactly, so it is not stored.
-template <int VARIANT, int VEC, bool ONEF = false>
+// SLAB: the stencils of the warped images are local to the slab (its outermost planes are halo and are discarded by
+// the caller); the static image is a whole volume, indexed in global planes.
+template <int VARIANT, int VEC, bool ONEF = false, bool SLAB = false>
 __global__ void __launch_bounds__(BX* BY) k_force_active(const KParams p0) {
     const unsigned b = blockIdx.z / (unsigned)p0.chunks, cz = blockIdx.z - b * (unsigned)p0.chunks;
     if (skip_pass(p0.sink, b)) return;
@@ -516,12 +569,15 @@ __global__ void __launch_bounds__(BX* BY) k_force_active(const KParams p0) {
     if (active) {
         for (int z = (int)cz * p.zper; z < min(d.nz, (int)(cz + 1) * p.zper); ++z) {
             const unsigned i0 = (unsigned)((z * d.ny + y) * d.nx + x0);
+            const int zoff = SLAB ? p.zoff : 0;
+            const Dims dg = SLAB ? Dims{d.nx, d.ny, p.gnz} : d;
+            const bool counted = !SLAB || (z >= p.mz0 && z < p.mz1);
             float mw[VEC], ax[VEC], ay[VEC], az[VEC];  // warped moving image and its gradient
             centre_and_gradient<VEC>(p.Mw, d, x0, y, z, mw, ax, ay, az);
             float fx[VEC], fy[VEC], fz[VEC], dd[VEC];
             if constexpr (VARIANT == 2) {  // Eq.(3)
                 float s[VEC];
-                load_vec<VEC>(p.S + i0, s);
+                load_vec<VEC>(p.S + (i0 + (unsigned)zoff * (unsigned)(d.nx * d.ny)), s);
 #pragma unroll
                 for (int j = 0; j < VEC; ++j) {
                     dd[j] = mw[j] - s[j];
@@ -532,7 +588,7 @@ __global__ void __launch_bounds__(BX* BY) k_force_active(const KParams p0) {
                 }
             } else if constexpr (VARIANT == 3 || VARIANT == 4) {  // Eq.(4), Eq.(5)
                 float s[VEC], gx[VEC], gy[VEC], gz[VEC];
-                centre_and_gradient<VEC>(p.S, d, x0, y, z, s, gx, gy, gz);
+                centre_and_gradient<VEC>(p.S, dg, x0, y, z + zoff, s, gx, gy, gz);
                 const float a2 = VARIANT == 4 ? p.alpha2 : 1.f;
 #pragma unroll
                 for (int j = 0; j < VEC; ++j) {
@@ -587,9 +643,11 @@ __global__ void __launch_bounds__(BX* BY) k_force_active(const KParams p0) {
                 store_vec<VEC>(p.ub_out + N + i0, uy);
                 store_vec<VEC>(p.ub_out + 2 * N + i0, uz);
             }
-            acc[0] += (double)ssd;
-            acc[1] += (double)sf;
-            acc[2] += (double)su;
+            if (counted) {
+                acc[0] += (double)ssd;
+                acc[1] += (double)sf;
+                acc[2] += (double)su;
+            }
         }
     }
     reduce_metrics(acc, p.sink, b, cz, (unsigned)p.chunks);
@@ -656,6 +714,10 @@ KParams make_params(const ForceArgs& a) {
     p.sink = a.sink;
     p.texM = a.texM;
     p.img_stride = (unsigned)a.img_stride;
+    p.zoff = a.slab ? a.zoff : 0;
+    p.gnz = a.slab ? a.gnz : a.d.nz;
+    p.mz0 = a.slab ? a.mz0 : 0;
+    p.mz1 = a.slab ? a.mz1 : a.d.nz;
     return p;
 }
 
@@ -695,17 +757,24 @@ int launch_lc(const ForceArgs& a, bool vec4, cudaStream_t st) {
         }
         cudaLaunchKernelEx(&cfg, kernel, p);
     };
+    constexpr bool S = !TEX;  // the z-slab instantiations exist for the software sampler only
     if (a.variant == 0) {
-        if (a.nb == 1) run(k_force_fixed_lc<0, XPT, FULL, TEX, MINB, false>);
+        if (a.slab) run(k_force_fixed_lc<0, XPT, FULL, TEX, MINB, false, S>);
+        else if (a.nb == 1) run(k_force_fixed_lc<0, XPT, FULL, TEX, MINB, false>);
         else run(k_force_fixed_lc<0, XPT, FULL, TEX, MINB, true>);
         return 1;
     }
     if (a.variant == 1) {
-        if (a.nb == 1) run(k_force_fixed_lc<1, XPT, FULL, TEX, MINB, false>);
+        if (a.slab) run(k_force_fixed_lc<1, XPT, FULL, TEX, MINB, false, S>);
+        else if (a.nb == 1) run(k_force_fixed_lc<1, XPT, FULL, TEX, MINB, false>);
         else run(k_force_fixed_lc<1, XPT, FULL, TEX, MINB, true>);
         return 1;
     }
-    if (a.variant == 5 && a.one_field) run(k_warp_lc<XPT, FULL, 2, TEX>);
+    if (a.slab) {
+        if (a.variant == 5 && a.one_field) run(k_warp_lc<XPT, FULL, 2, TEX, S>);
+        else if (a.variant == 5) run(k_warp_lc<XPT, FULL, 1, TEX, S>);
+        else run(k_warp_lc<XPT, FULL, 0, TEX, S>);
+    } else if (a.variant == 5 && a.one_field) run(k_warp_lc<XPT, FULL, 2, TEX>);
     else if (a.variant == 5) run(k_warp_lc<XPT, FULL, 1, TEX>);
     else run(k_warp_lc<XPT, FULL, 0, TEX>);
     if (a.ev_mid) cudaEventRecord(a.ev_mid, st);
@@ -718,6 +787,22 @@ int launch_lc(const ForceArgs& a, bool vec4, cudaStream_t st) {
         p.chunks = (a.d.nz + sh.zper - 1) / sh.zper;
         kernel<<<dim3(tx, (a.d.ny + BY - 1) / BY, p.chunks * a.nb), dim3(BX, BY), 0, st>>>(p);
     };
+    if (a.slab) {
+        switch (a.variant) {
+        case 2: if (vec4) run_active(k_force_active<2, 4, false, true>); else run_active(k_force_active<2, 1, false, true>); break;
+        case 3: if (vec4) run_active(k_force_active<3, 4, false, true>); else run_active(k_force_active<3, 1, false, true>); break;
+        case 4: if (vec4) run_active(k_force_active<4, 4, false, true>); else run_active(k_force_active<4, 1, false, true>); break;
+        case 5:
+            if (a.one_field) {
+                if (vec4) run_active(k_force_active<5, 4, true, true>); else run_active(k_force_active<5, 1, true, true>);
+            } else {
+                if (vec4) run_active(k_force_active<5, 4, false, true>); else run_active(k_force_active<5, 1, false, true>);
+            }
+            break;
+        default: return -1;
+        }
+        return 2;
+    }
     switch (a.variant) {
     case 2: if (vec4) run_active(k_force_active<2, 4>); else run_active(k_force_active<2, 1>); break;
     case 3: if (vec4) run_active(k_force_active<3, 4>); else run_active(k_force_active<3, 1>); break;
@@ -819,10 +904,27 @@ int force_partial_blocks(const Dims& d) {
     return (int)(n > generic ? n : generic);
 }
 
-int launch_grad_mag2(const Dims& d, const float* I, size_t img_stride, float* out, int nb, cudaStream_t st) {
-    if ((long long)d.nz * nb > 65535) return -1;
-    const dim3 grid((d.nx + 63) / 64, (d.ny + 3) / 4, d.nz * nb);
-    k_grad_mag2<<<grid, dim3(64, 4), 0, st>>>(I, out, d, img_stride);
+int launch_grad_mag2(const Dims& d, const float* I, size_t img_stride, float* out, int nb, cudaStream_t st, int z0,
+                     int zn) {
+    if (zn < 0) zn = d.nz - z0;  // default: every plane
+    if (z0 < 0 || zn < 1 || z0 + zn > d.nz) return -1;
+    if (d.nx % 4 == 0 && aligned16(I) && aligned16(out) && (nb == 1 || img_stride % 4 == 0)) {
+        // enough z chunks for about four blocks per SM
+        const long long xy = (long long)((d.nx / 4 + 31) / 32) * ((d.ny + 7) / 8) * nb;
+        long long chunks = (4LL * sm_count() + xy - 1) / xy;
+        if (chunks > zn) chunks = zn;
+        if (chunks < 1) chunks = 1;
+        const int zper = (int)((zn + chunks - 1) / chunks);
+        chunks = (zn + zper - 1) / zper;
+        if (chunks * nb <= 65535) {
+            const dim3 grid((d.nx / 4 + 31) / 32, (d.ny + 7) / 8, (unsigned)(chunks * nb));
+            k_grad_mag2_v4<<<grid, dim3(32, 8), 0, st>>>(I, out, d, img_stride, zper, (int)chunks, z0, zn);
+            return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+        }
+    }
+    if ((long long)zn * nb > 65535) return -1;
+    const dim3 grid((d.nx + 63) / 64, (d.ny + 3) / 4, zn * nb);
+    k_grad_mag2<<<grid, dim3(64, 4), 0, st>>>(I, out, d, img_stride, z0, zn);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
@@ -835,6 +937,7 @@ int launch_negate(const float* in, float* out, size_t n, cudaStream_t st) {
 
 int launch_warp_force(const ForceArgs& a, cudaStream_t st) {
     if (a.nb < 1 || (a.texM != 0 && a.nb != 1)) return -1;
+    if (a.slab && (a.nb != 1 || a.texM != 0 || a.d.nx < 2 || a.d.ny < 2 || a.d.nz < 2 || a.gnz < 2)) return -1;
     const bool vec4 = (a.d.nx % 4 == 0) && aligned16(a.S) && aligned16(a.M) && aligned16(a.u_in) &&
                       aligned16(a.u_out) && aligned16(a.ub_in) && aligned16(a.ub_out) && aligned16(a.Mw) &&
                       aligned16(a.Sw) && (a.nb == 1 || (a.img_stride % 4 == 0 && nvox(a.d) % 4 == 0));

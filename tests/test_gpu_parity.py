@@ -433,6 +433,60 @@ def test_inverse_consistent_one_field_is_bit_identical(torch_cuda, B, P, oracle)
     eng.close()
 
 
+@pytest.mark.parametrize("variant,world,levels", [(0, 3, 1), (1, 2, 1), (2, 3, 1), (3, 2, 2), (5, 2, 1), (0, 4, 2)])
+def test_z_slab_decomposition_is_bit_identical(torch_cuda, B, P, variant, world, levels):
+    """the registration split into z slabs (own planes + R + 1 halo planes, images replicated, one
+    halo refresh per iteration; paper_0909_0928_b200/slabs.py) gives on every rank's own planes the bits of the
+    undivided registration.  The ranks are emulated one after another on this GPU; their halos move through
+    LocalExchange, the same bookkeeping DistExchange does over NCCL."""
+    torch = torch_cuda
+    from paper_0909_0928_b200 import slabs as SL
+    dims = (64, 40, 44)
+    sigma = 1.0
+    alpha = ALPHA.get(variant, 1.0)
+    S, M, _ = P.config1_pair(dims=dims, seed=55, max_norm=2.5)
+    iters = [7, 6][-levels:] if levels == 2 else [6]
+    ic = variant == 5
+    dS, dM = dev(torch, S), dev(torch, M)
+    # the undivided registration (graphs off: the slab loop launches kernel by kernel as well)
+    eng = B.Demons(dims, variant=variant, alpha=alpha, sigma=sigma, levels=levels)
+    B.demons_set_option(eng.ctx, "ic_one_field", 0)
+    if levels == 1:
+        B.demons_set_option(eng.ctx, "zero_start", 1)
+    du = torch.zeros((3,) + S.shape, dtype=torch.float32, device="cuda:0")
+    dub = torch.zeros_like(du) if ic else None
+    stats = np.zeros((int(sum(iters)), 3))
+    B.demons_register(eng.ctx, dS, dM, du, dub, iters, 0.0, stats, None, None)
+    torch.cuda.synchronize()
+    eng.close()
+    # the same in `world` slabs
+    plan = SL.plan(dims[2], world, SL.halo_planes(sigma))
+    assert plan[0].lo == 0 and plan[-1].hi == dims[2] and all(a.own1 == b.own0 for a, b in zip(plan, plan[1:]))
+    if levels == 2:
+        u0, ub0 = SL.coarse_levels_replicated(dims, (1.0, 1.0, 1.0), variant, alpha, sigma, dS, dM, iters[:-1], "cuda:0")
+    else:
+        u0 = torch.zeros_like(du)
+        ub0 = torch.zeros_like(du) if ic else None
+    engines = [B.Demons(dims, variant=variant, alpha=alpha, sigma=sigma, levels=1) for _ in plan]
+    fields = [u0[:, s.lo:s.hi].contiguous() for s in plan]
+    scratch = [torch.empty_like(f) for f in fields]
+    fields_b = [ub0[:, s.lo:s.hi].contiguous() for s in plan] if ic else None
+    scratch_b = [torch.empty_like(f) for f in fields_b] if ic else None
+    metrics = [torch.zeros((iters[-1], 3), dtype=torch.float64, device="cuda:0") for _ in plan]
+    SL.iterate_slabs(engines, plan, dS, dM, fields, scratch, iters[-1], sigma, SL.LocalExchange(plan), metrics,
+                     fields_b, scratch_b)
+    torch.cuda.synchronize()
+    for s in plan:
+        own = fields[s.rank][:, s.own_begin:s.own_begin + s.own_count]
+        assert torch.equal(own, du[:, s.own0:s.own1]), f"rank {s.rank} of {world}"
+        if ic:
+            assert torch.equal(fields_b[s.rank][:, s.own_begin:s.own_begin + s.own_count], dub[:, s.own0:s.own1])
+    total = sum(m.cpu().numpy() for m in metrics)          # the all-reduce of the three sums
+    np.testing.assert_allclose(total, stats[-iters[-1]:], rtol=1e-12)
+    for e in engines:
+        e.close()
+
+
 def test_api_rejects_bad_calls(torch_cuda, B):
     torch = torch_cuda
     dims = (16, 16, 8)

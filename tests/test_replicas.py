@@ -69,3 +69,55 @@ def test_bench_spawns_its_own_ranks():
     assert line["n_gpus"] == 2 and line["units"] == 6.0
     # max over ranks: rank 1 sleeps 20 ms per step
     assert line["ms_per_step"] >= 19.0
+
+
+def test_slab_plan_covers_the_volume():
+    from paper_0909_0928_b200 import slabs as SL
+    assert SL.halo_planes(1.0) == 4 and SL.halo_planes(2.0) == 7
+    for nz, world in ((256, 8), (100, 3), (44, 4), (37, 2), (9, 1)):
+        plan = SL.plan(nz, world, 4)
+        assert plan[0].own0 == 0 and plan[-1].own1 == nz
+        for a, b in zip(plan, plan[1:]):
+            assert a.own1 == b.own0                      # own ranges tile the volume
+            assert a.hi == a.own1 + 4 and b.lo == b.own0 - 4
+        assert plan[0].lo == 0 and plan[-1].hi == nz     # no halo beyond a face of the volume
+        assert max(s.own_count for s in plan) - min(s.own_count for s in plan) <= 1
+    with pytest.raises(ValueError):
+        SL.plan(12, 4, 4)                                # 3 planes per rank cannot fill a 4-plane halo
+
+
+def _slab_worker(rank, world, port, out):
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port))
+    import torch
+    import torch.distributed as dist
+    from paper_0909_0928_b200 import replicas, slabs as SL
+    replicas.init("gloo")
+    nz, ny, nx, halo = 23, 3, 5, 4
+    s = SL.plan(nz, world, halo)[rank]
+    # the "field": plane z of component c holds 100 c + z on own planes, -1 in the halos
+    f = torch.full((3, s.count, ny, nx), -1.0)
+    for c in range(3):
+        for z in range(s.own0, s.own1):
+            f[c, z - s.lo] = 100.0 * c + z
+    SL.DistExchange(s).refresh(f)
+    want = torch.stack([torch.stack([torch.full((ny, nx), 100.0 * c + z) for z in range(s.lo, s.hi)]) for c in range(3)])
+    out.put((rank, bool(torch.equal(f, want))))
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_slab_halo_exchange_over_gloo(world):
+    """DistExchange (the NCCL path's bookkeeping) on CPU: after one refresh every halo plane holds the
+    neighbour's own plane."""
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_slab_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert res == [(r, True) for r in range(world)]
