@@ -180,7 +180,9 @@ int demons_warp_force(demons_ctx* ctx, const int dims[3], const float* d_static,
  * [warp_force_slab ; demons_smooth on the slab] exact on the own planes; the caller then refreshes the halos from
  * the neighbours' own planes (paper_0909_0928_b200/slabs.py: torch.distributed send/recv, one exchange per
  * iteration).  d_metrics (nullable): the three sums over planes [own_begin, own_begin + own_count) of the SLAB
- * (local indices), to be added over the ranks.  The context must have been created with the whole volume's dims;
+ * (local indices), to be added over the ranks.  Variant 5 with d_ub_in = d_ub_out = NULL is the one-field form: the
+ * caller holds u_b = -u_f (exact from a zero start, "ic_one_field") and S is warped by -u_f.
+ * The context must have been created with the whole volume's dims;
  * z_count >= 2.  The "texture" option is not served. */
 int demons_warp_force_slab(demons_ctx* ctx, const int dims[3], int z_begin, int z_count, int own_begin, int own_count,
                            const float* d_static, const float* d_moving, const float* d_u_in, float* d_u_out,

@@ -829,7 +829,9 @@ int demons_warp_force_slab(demons_ctx* c, const int dims[3], int z_begin, int z_
     if (!d_static || !d_moving || !d_u_in || !d_u_out) return fail(DEMONS_E_ARG, "NULL volume / field pointer");
     if (d_u_in == d_u_out) return fail(DEMONS_E_ARG, "u_out must not alias u_in");
     const bool ic = is_ic(c);
-    if (ic && (!d_ub_in || !d_ub_out)) return fail(DEMONS_E_ARG, "variant 5 needs ub_in and ub_out");
+    // variant 5 without the backward field: the one-field form (the caller holds u_b = -u_f, pin P10)
+    const bool one_field = ic && !d_ub_in && !d_ub_out;
+    if (ic && !one_field && (!d_ub_in || !d_ub_out)) return fail(DEMONS_E_ARG, "variant 5 needs both ub_in and ub_out, or neither");
     if (!ic && (d_ub_in || d_ub_out)) return fail(DEMONS_E_ARG, "ub_in / ub_out must be NULL unless variant 5");
     if (c->opt_texture) return fail(DEMONS_E_UNSUPPORTED, "the texture option serves whole volumes only");
     rc = check_ws(c, 1);
@@ -851,6 +853,7 @@ int demons_warp_force_slab(demons_ctx* c, const int dims[3], int z_begin, int z_
     fa.Mw = reinterpret_cast<float*>(c->ws + p.Mw);  // variant 1: |grad M|^2 in GLOBAL indexing; else the slab's Mw
     fa.Sw = ic ? reinterpret_cast<float*>(c->ws + p.Sw) : nullptr;
     fa.sink = make_sink(c, p, 0, d_metrics, 0, false, 0.0);
+    fa.one_field = one_field ? 1 : 0;
     fa.slab = 1;
     fa.zoff = z_begin;
     fa.gnz = g.nz;
