@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(BX* BY) k_force_fixed(const KParams p0) {
                     const float dd = mw[j] - s[j];
                     const float s2 = fmaf(gx[j], gx[j], fmaf(gy[j], gy[j], gz[j] * gz[j]));
                     const float m2 = fmaf(hx[j], hx[j], fmaf(hy[j], hy[j], hz[j] * hz[j]));
-                    const float num = 4.f * dd * fast_sqrt(s2) * fast_sqrt(m2);
+                    const float num = 4.f * dd * fast_sqrt(s2 * m2);  // |gS| |gM0| with one square root
                     const float den = (fmaf(2.f * dd, dd, s2 + m2)) * (s2 + m2);
                     k[j] = guarded_div(num, den);
                 }
@@ -358,7 +358,7 @@ __global__ void __launch_bounds__(BX* BY, MINB) k_force_fixed_lc(const KParams p
                     // Eq.(2) needs only |gM0|, the gradient magnitude of the UNWARPED level moving image at the grid
                     // point (reading A4): fixed for the level, so it is read from a precomputed volume
                     const float m2 = q.m2[j];
-                    const float num = 4.f * dd * fast_sqrt(g2) * fast_sqrt(m2);
+                    const float num = 4.f * dd * fast_sqrt(g2 * m2);  // |gS| |gM0| with one square root
                     const float den = (fmaf(2.f * dd, dd, g2 + m2)) * (g2 + m2);
                     k = guarded_div(num, den);
                 }

@@ -107,3 +107,40 @@ def test_options_are_host_only_and_validated(B):
             B.demons_set_option(ctx, "no_such_option", 1)
     finally:
         B.demons_destroy(ctx)
+
+
+def test_batch_and_slab_arguments_validated(B):
+    """Host-side validation of the batched and the z-slab entry points (no device needed)."""
+    import numpy as np
+    dims = (16, 12, 10)
+    ctx = B.demons_create(dims, (1.0, 1.0, 1.0), B.PASSIVE, 1.0, 1.0)
+    try:
+        w1, w4 = B.demons_workspace_bytes_batch(ctx, 2, 1), B.demons_workspace_bytes_batch(ctx, 2, 4)
+        assert w1 == B.demons_workspace_bytes(ctx, 2) and w4 > 3 * (w1 - 5 * 4 * 16 * 12 * 10)
+        assert B.demons_workspace_bytes_batch(ctx, 2, 0) == 0 and B.demons_workspace_bytes_batch(ctx, 2, 65) == 0
+        vol = np.zeros((4, 10, 12, 16), np.float32)
+        fld = np.zeros((4, 3, 10, 12, 16), np.float32)
+        for nb in (0, 65):
+            with pytest.raises(B.DemonsError) as e:
+                B.demons_register_batch(ctx, nb, vol, vol, fld, None, [2, 2])
+            assert e.value.code == B.E_ARG
+        with pytest.raises(B.DemonsError) as e:
+            B.demons_register_batch(ctx, 4, vol, vol, fld, fld, [2, 2])      # u_back for a non-IC variant
+        assert e.value.code == B.E_ARG
+        with pytest.raises(B.DemonsError) as e:
+            B.demons_register_batch(ctx, 4, vol, vol, fld, None, [2, 2])     # valid arguments, but no workspace / device
+        assert e.value.code == B.E_WORKSPACE
+        slab = np.zeros((3, 6, 12, 16), np.float32)
+        bad = [dict(z_begin=-1), dict(z_begin=6, z_count=6), dict(z_count=1), dict(own_begin=5, own_count=3), dict(own_count=-1)]
+        for kw in bad:
+            a = dict(z_begin=2, z_count=6, own_begin=1, own_count=4)
+            a.update(kw)
+            with pytest.raises(B.DemonsError) as e:
+                B.demons_warp_force_slab(ctx, dims, a["z_begin"], a["z_count"], a["own_begin"], a["own_count"], vol[0], vol[0],
+                                         slab, slab.copy())
+            assert e.value.code == B.E_ARG, kw
+        with pytest.raises(B.DemonsError) as e:
+            B.demons_warp_force_slab(ctx, dims, 2, 6, 1, 4, vol[0], vol[0], slab, slab)   # aliased output
+        assert e.value.code == B.E_ARG
+    finally:
+        B.demons_destroy(ctx)
