@@ -16,9 +16,17 @@
 // clamped when the shared-memory addresses are formed.
 // HBM sees every element once in and once out (8 B / element); the paper's design was one
 // kernel per axis through shared memory (L175), i.e. 24 B / element.
+// R >= 5 (one CTA per SM): work is split evenly over ONE wave of CTAs (round 2): the columns (tile, component) are laid end to end on a
+// virtual z axis, each preceded by its 2R warm-up planes, and CTA i takes the i-th equal share of that axis -- a
+// run of planes that may end one column and begin the next.  Equal z chunks cost  waves x (planes + 2R)  and left
+// half of the last wave idle at 256x256x100; the shares cost  total / slots + 2R  (70.2 -> 66.5 us there, 381 -> 346 us
+// at 512x512x160).  R <= 4 keeps equal chunks: with three CTAs per SM the even split gains 1.5 % standalone, and it
+// loses the reuse of the y halo rows between neighbouring tiles in L2 (204 -> 282 us at 512x512x160).
 // The march runs DOWN the z axis by default (`rev`): the force kernels march up, so the planes they
 // wrote last are read first while they are still in L2, and the planes written last here are the
 // ones the next force kernel reads first.  The taps are symmetric: the result is bit-identical.
+#include <algorithm>
+
 #include "kernels.h"
 #include "tma.cuh"
 
@@ -67,10 +75,10 @@ struct Cfg {
     static_assert(PAIR == 1 || (PAIR == 2 && STAGES % 2 == 0), "pairs need an even number of stages");
 };
 
-template <int R, int K, int RG, int STAGES, int MINB, int PAIR>
+template <int R, int K, int RG, int STAGES, int MINB, int PAIR, int XP, int BAL>
 __global__ void __launch_bounds__(32 * (RG + 1), MINB)
     k_smooth_tma(const __grid_constant__ CUtensorMap tmap, float* __restrict__ out, const Dims d, const int zc,
-                 const int tiles_x, const Taps t, const Control* __restrict__ ctl, const int comps_per_pair, const int rev) {
+                 const int tiles_x, const Taps t, const Control* __restrict__ ctl, const int comps_per_pair, const int rev, const int tiles, const int ncols) {
     using C = Cfg<R, K, RG, STAGES, PAIR>;
     constexpr int LR = C::LR;
     constexpr int NH = C::NH, L = C::L, GX = C::GX, GW = C::GW, TY = C::TY, BOXW = C::BOXW;
@@ -78,18 +86,37 @@ __global__ void __launch_bounds__(32 * (RG + 1), MINB)
     float4* xs = reinterpret_cast<float4*>(smem + STAGES * C::STAGE_BYTES);  // [2][TY][GW]
     uint64_t* full = reinterpret_cast<uint64_t*>(smem + STAGES * C::STAGE_BYTES + C::XS_BYTES);
 
-    // the stopping rule of this component's pair has fired (PAPER.md L145): nothing to do
-    if (ctl != nullptr && *reinterpret_cast<const volatile int*>(&ctl[blockIdx.z / comps_per_pair].stop_smooth) != 0) return;
+    if constexpr (!BAL) {
+        // the stopping rule of this component's pair has fired: nothing to do
+        if (ctl != nullptr && *reinterpret_cast<const volatile int*>(&ctl[blockIdx.z / comps_per_pair].stop_smooth) != 0) return;
+    }
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const bool halo_warp = warp == RG;
-    const int tile_x = blockIdx.x % tiles_x, tile_y = blockIdx.x / tiles_x;
-    const int x0 = tile_x * GX * 4, y0 = tile_y * TY;
-    const int comp = blockIdx.z;
-    const int z_start = blockIdx.y * zc;
-    const int nplanes = min(zc, d.nz - z_start);
-    const int P = nplanes + 2 * R;
     const size_t plane = (size_t)d.nx * d.ny;
+    const bool issuer = halo_warp && lane == 0;
+
+    // BAL: this CTA's share [va, vb) of the virtual axis -- column c occupies [c W, (c + 1) W), W = nz + 2R, and position
+    // c W + 2R + z is output plane z of that column.  Otherwise: grid (tile, z chunk, component), one segment per CTA
+    // (this loop runs once and folds away).
+    const int W = d.nz + 2 * R;
+    int col_first = 0, col_last = 0, off_a = 0, off_b = 0;
+    if constexpr (BAL) {
+        const long long V = (long long)ncols * W;
+        const long long va = V * blockIdx.x / gridDim.x, vb = V * (blockIdx.x + 1) / gridDim.x;
+        col_first = (int)(va / W), col_last = (int)((vb - 1) / W);
+        off_a = (int)(va - (long long)col_first * W), off_b = (int)(vb - (long long)col_last * W);
+    }
+    bool bars_live = false;
+
+    // one segment: planes [z_start, z_start + nplanes) of column (tile, comp), warm-up included
+    auto segment = [&](const int z_start, const int nplanes, const int comp, const int tile) {
+    if (nplanes <= 0) return;  // the share ends inside the warm-up prefix of this column
+    // the stopping rule of this component's pair has fired (PAPER.md L145): nothing to do
+    if (BAL && ctl != nullptr && *reinterpret_cast<const volatile int*>(&ctl[comp / comps_per_pair].stop_smooth) != 0) return;
+    const int tile_x = tile % tiles_x, tile_y = tile / tiles_x;
+    const int x0 = tile_x * GX * 4, y0 = tile_y * TY;
+    const int P = nplanes + 2 * R;
 
     // role of this thread: which float4 group (g) of which row group (rg)
     int g, rg;
@@ -120,18 +147,24 @@ __global__ void __launch_bounds__(32 * (RG + 1), MINB)
 #pragma unroll
     for (int k = 0; k <= R; ++k) w2[k] = make_float2(t.w[k], t.w[k]);
 
-    const bool issuer = halo_warp && lane == 0;
     auto issue = [&](int p) {  // plane p of the march -> stage p % STAGES
         const int s = p % STAGES;
         const int z = min(max(rev ? z_start + nplanes - 1 + R - p : z_start - R + p, 0), d.nz - 1);
         mbar_expect_tx(&full[s], (uint32_t)(C::ROWS * BOXW * 4));
         tma::load_4d(smem + s * C::STAGE_BYTES, &tmap, &full[s], x0 - 4 * NH, y0 - R, z, comp);
     };
+    // a segment starts with fresh barriers (phase 0), so that stage and parity of plane p stay p % STAGES and
+    // (p / STAGES) & 1; the __syncthreads also keeps a fast warp out of the exchange buffer the slow ones still read
+    if constexpr (BAL) __syncthreads();
     if (issuer) {
 #pragma unroll
-        for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 1);
+        for (int s = 0; s < STAGES; ++s) {
+            if (BAL && bars_live) tma::mbar_inval(&full[s]);
+            mbar_init(&full[s], 1);
+        }
         tma::mbar_fence_init();
     }
+    bars_live = true;
     __syncthreads();
     if (issuer) {
         for (int p = 0; p < STAGES && p < P; ++p) issue(p);
@@ -168,13 +201,89 @@ __global__ void __launch_bounds__(32 * (RG + 1), MINB)
                 }
                 ys[j].a = a;
                 ys[j].b = b;
-                xrow[j * GW + g] = make_float4(a.x, a.y, b.x, b.y);
+                if constexpr (!XP) xrow[j * GW + g] = make_float4(a.x, a.y, b.x, b.y);
+            }
+            if constexpr (XP) {  // rows 2jp and 2jp + 1 interleaved element by element: (r0 x0, r1 x0, r0 x1, r1 x1), (.. x2, x3)
+#pragma unroll
+                for (int jp = 0; jp < K / 2; ++jp) {
+                    const F4 &r0 = ys[2 * jp], &r1 = ys[2 * jp + 1];
+                    xrow[(2 * jp) * GW + g] = make_float4(r0.a.x, r1.a.x, r0.a.y, r1.a.y);
+                    xrow[(2 * jp + 1) * GW + g] = make_float4(r0.b.x, r1.b.x, r0.b.y, r1.b.y);
+                }
+            }
+        }
+    };
+    // ---- x and z pass, ROW-PAIR form (XP; R >= 5).  Element e of the x window is the float2 (row 2jp, row 2jp + 1) at
+    // one x, so every tap is an aligned register pair and the whole x pass is packed f32x2 (half the instructions of
+    // the scalar pass; the y pass wrote the exchange rows interleaved that way).  The ring and the z pass carry the
+    // same pairs; the rows are separated again at the store.
+    auto xzpass_xp = [&](int p, int sl, const F4 (&ys)[K], const float4* xrow) {
+        static_assert(!XP || K % 2 == 0, "row pairs");
+        float4 q[K][2 * NH];  // the neighbours' y-smoothed float4s of this thread's exchange rows
+#pragma unroll
+        for (int r = 0; r < K; ++r)
+#pragma unroll
+            for (int h = 0; h < 2 * NH; ++h) q[r][h] = xrow[r * GW + g - NH + (h < NH ? h : h + 1)];
+#pragma unroll
+        for (int jp = 0; jp < K / 2; ++jp) {
+            float2 a[4 * (2 * NH + 1)];
+#pragma unroll
+            for (int h = 0; h < 2 * NH + 1; ++h) {
+                if (h == NH) {
+                    const F4 &r0 = ys[2 * jp], &r1 = ys[2 * jp + 1];
+                    a[4 * h + 0] = make_float2(r0.a.x, r1.a.x);
+                    a[4 * h + 1] = make_float2(r0.a.y, r1.a.y);
+                    a[4 * h + 2] = make_float2(r0.b.x, r1.b.x);
+                    a[4 * h + 3] = make_float2(r0.b.y, r1.b.y);
+                } else {
+                    const float4 q0 = q[2 * jp][h < NH ? h : h - 1], q1 = q[2 * jp + 1][h < NH ? h : h - 1];
+                    a[4 * h + 0] = make_float2(q0.x, q0.y);
+                    a[4 * h + 1] = make_float2(q0.z, q0.w);
+                    a[4 * h + 2] = make_float2(q1.x, q1.y);
+                    a[4 * h + 3] = make_float2(q1.z, q1.w);
+                }
+            }
+            float2 o[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                float2 acc = __fmul2_rn(w2[0], a[4 * NH + e]);
+#pragma unroll
+                for (int k = 1; k <= R; ++k) acc = __ffma2_rn(w2[k], __fadd2_rn(a[4 * NH + e - k], a[4 * NH + e + k]), acc);
+                o[e] = acc;
+            }
+            ring[sl][2 * jp].a = o[0];  // (x0, x1) of the row pair
+            ring[sl][2 * jp].b = o[1];
+            ring[sl][2 * jp + 1].a = o[2];  // (x2, x3)
+            ring[sl][2 * jp + 1].b = o[3];
+        }
+        if (p >= 2 * R) {
+            float* orow = dst + (size_t)(rev ? z_start + nplanes - 1 - (p - 2 * R) : z_start + p - 2 * R) * plane;
+            F4 zo[K];
+#pragma unroll
+            for (int j = 0; j < K; ++j) {
+                const F4& c = ring[(sl - R + LR) % LR][j];
+                float2 a = __fmul2_rn(w2[0], c.a), b = __fmul2_rn(w2[0], c.b);
+#pragma unroll
+                for (int k = 1; k <= R; ++k) {
+                    const F4& lo = ring[(sl - R - k + 2 * LR) % LR][j];
+                    const F4& hi = ring[(sl - R + k + LR) % LR][j];
+                    a = __ffma2_rn(w2[k], __fadd2_rn(lo.a, hi.a), a);
+                    b = __ffma2_rn(w2[k], __fadd2_rn(lo.b, hi.b), b);
+                }
+                zo[j].a = a;
+                zo[j].b = b;
+            }
+#pragma unroll
+            for (int j = 0; j < K; ++j) {  // .x = even row, .y = odd row
+                const F4 &lo = zo[j & ~1], &hi = zo[j | 1];
+                const float4 v = (j & 1) ? make_float4(lo.a.y, lo.b.y, hi.a.y, hi.b.y) : make_float4(lo.a.x, lo.b.x, hi.a.x, hi.b.x);
+                if (y0 + rg * K + j < d.ny) *reinterpret_cast<float4*>(orow + (size_t)j * d.nx) = v;
             }
         }
     };
     // ---- x pass of plane p into ring slot sl (neighbours' float4s from the exchange buffer), then the
     // z pass of the plane R behind it (register ring, packed f32x2) and its store
-    auto xzpass = [&](int p, int sl, const F4 (&ys)[K], const float4* xrow) {
+    auto xzpass_scalar = [&](int p, int sl, const F4 (&ys)[K], const float4* xrow) {
 #pragma unroll
         for (int j = 0; j < K; ++j) {
             float a[4 * (2 * NH + 1)];
@@ -233,7 +342,10 @@ __global__ void __launch_bounds__(32 * (RG + 1), MINB)
                     ypass(p, ys, xrow);
                     __syncthreads();  // xs complete; every warp is done reading this raw stage
                     if (issuer && p + STAGES < P) issue(p + STAGES);
-                    if (owner) xzpass(p, s, ys, xrow);
+                    if (owner) {
+                        if constexpr (XP) xzpass_xp(p, s, ys, xrow);
+                        else xzpass_scalar(p, s, ys, xrow);
+                    }
                 }
             }
         }
@@ -257,47 +369,23 @@ __global__ void __launch_bounds__(32 * (RG + 1), MINB)
                         if (p0 + 1 + STAGES < P) issue(p0 + 1 + STAGES);
                     }
                     if (owner) {
-                        xzpass(p0, 2 * s2, ys0, xr0);
-                        if (two) xzpass(p0 + 1, 2 * s2 + 1, ys1, xr1);
+                        xzpass_scalar(p0, 2 * s2, ys0, xr0);
+                        if (two) xzpass_scalar(p0 + 1, 2 * s2 + 1, ys1, xr1);
                     }
                 }
             }
         }
     }
-}
-
-template <int R, int K, int RG, int STAGES, int MINB, int PAIR = 1>
-int launch_cfg(const SmoothArgs& a, int zc, cudaStream_t st) {
-    using C = Cfg<R, K, RG, STAGES, PAIR>;
-    const Dims d = a.d;
-    alignas(64) CUtensorMap map;
-    const unsigned long long gdim[4] = {(unsigned long long)d.nx, (unsigned long long)d.ny, (unsigned long long)d.nz,
-                                        (unsigned long long)a.ncomp};
-    const unsigned box[4] = {(unsigned)C::BOXW, (unsigned)C::ROWS, 1u, 1u};
-    if (!tma::encode_f32(&map, a.in, 4, gdim, box)) return 0;
-    static bool attr_set[64] = {};  // per device: the attribute belongs to the device's copy of the kernel
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 0;
-    if (!attr_set[dev]) {
-        if (cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES, MINB, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM) !=
-            cudaSuccess) {
-            cudaGetLastError();
-            return 0;  // refused: not applicable here, the caller falls back to the separable passes
+    };  // segment
+    if constexpr (BAL) {
+        for (int col = col_first; col <= col_last; ++col) {
+            const int z_start = col == col_first ? max(off_a - 2 * R, 0) : 0;
+            const int z_end = col == col_last ? min(off_b - 2 * R, d.nz) : d.nz;
+            segment(z_start, z_end - z_start, col / tiles, col % tiles);
         }
-        cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES, MINB, PAIR>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-        attr_set[dev] = true;
+    } else {
+        segment(blockIdx.y * zc, min(zc, d.nz - (int)blockIdx.y * zc), blockIdx.z, blockIdx.x);
     }
-    const int tiles_x = (d.nx + C::GX * 4 - 1) / (C::GX * 4);
-    const int tiles_y = (d.ny + C::TY - 1) / C::TY;
-    const int chunks = (d.nz + zc - 1) / zc;
-    if (chunks > 65535 || a.ncomp > 65535) return 0;
-    Taps t;
-    for (int k = 0; k < 8; ++k) t.w[k] = k <= a.R ? a.w[k] : 0.f;
-    const dim3 grid(tiles_x * tiles_y, chunks, a.ncomp);
-    k_smooth_tma<R, K, RG, STAGES, MINB, PAIR><<<grid, C::THREADS, C::SMEM, st>>>(map, a.out, d, zc, tiles_x, t, a.ctl,
-                                                                             a.comps_per_pair > 0 ? a.comps_per_pair : a.ncomp,
-                                                                             a.ascending ? 0 : 1);
-    return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
 // Planes per CTA: the number of z chunks that minimises  waves x (planes per chunk + 2R warm-up).
@@ -319,6 +407,50 @@ int pick_zc(const SmoothArgs& a, int tile_w, int tile_h, int slots) {
     return best_zc;
 }
 
+template <int R, int K, int RG, int STAGES, int MINB, int PAIR = 1, int XP = 0, int BAL = 0>
+int launch_cfg(const SmoothArgs& a, int slots, cudaStream_t st) {
+    using C = Cfg<R, K, RG, STAGES, PAIR>;
+    const Dims d = a.d;
+    alignas(64) CUtensorMap map;
+    const unsigned long long gdim[4] = {(unsigned long long)d.nx, (unsigned long long)d.ny, (unsigned long long)d.nz,
+                                        (unsigned long long)a.ncomp};
+    const unsigned box[4] = {(unsigned)C::BOXW, (unsigned)C::ROWS, 1u, 1u};
+    if (!tma::encode_f32(&map, a.in, 4, gdim, box)) return 0;
+    static bool attr_set[64] = {};  // per device: the attribute belongs to the device's copy of the kernel
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 0;
+    if (!attr_set[dev]) {
+        if (cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES, MINB, PAIR, XP, BAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM) !=
+            cudaSuccess) {
+            cudaGetLastError();
+            return 0;  // refused: not applicable here, the caller falls back to the separable passes
+        }
+        cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES, MINB, PAIR, XP, BAL>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        attr_set[dev] = true;
+    }
+    const int tiles_x = (d.nx + C::GX * 4 - 1) / (C::GX * 4);
+    const int tiles_y = (d.ny + C::TY - 1) / C::TY;
+    const long long ncols = (long long)tiles_x * tiles_y * a.ncomp;
+    if (ncols * (d.nz + 2 * R) >= (1ll << 31)) return 0;
+    dim3 grid;
+    int zc = 0;
+    if constexpr (BAL) {
+        // one wave of equal shares; a share is never shorter than the 2R + 2 planes of a warm-up
+        grid = dim3((unsigned)std::max(1ll, std::min((long long)slots, ncols * (d.nz + 2 * R) / (2 * R + 2))));
+    } else {
+        zc = pick_zc(a, C::GX * 4, C::TY, slots);
+        const int chunks = (d.nz + zc - 1) / zc;
+        if (chunks > 65535 || a.ncomp > 65535) return 0;
+        grid = dim3(tiles_x * tiles_y, chunks, a.ncomp);
+    }
+    Taps t;
+    for (int k = 0; k < 8; ++k) t.w[k] = k <= a.R ? a.w[k] : 0.f;
+    k_smooth_tma<R, K, RG, STAGES, MINB, PAIR, XP, BAL><<<grid, C::THREADS, C::SMEM, st>>>(
+        map, a.out, d, zc, tiles_x, t, a.ctl, a.comps_per_pair > 0 ? a.comps_per_pair : a.ncomp,
+        a.ascending ? 0 : 1, tiles_x * tiles_y, (int)ncols);
+    return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+}
+
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 }  // namespace
@@ -327,20 +459,20 @@ bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) ==
 int launch_smooth_tma(const SmoothArgs& a, cudaStream_t st) {
     if (a.d.nx % 4 != 0 || a.d.nx < 4 || !aligned16(a.in) || !aligned16(a.out)) return 0;
     if (a.R < 1 || a.R > 6) return 0;
-    // (tile height, CTAs per SM) of the configuration picked below
-    int tile_h = 8, per_sm = 3;
+    // CTAs per SM of the configuration picked below (its launch bounds): the grid is one wave of them
+    int per_sm = 3;
     if (a.R == 4) per_sm = 2;
-    if (a.R > 4) tile_h = 16, per_sm = 1;
-    const int zc = pick_zc(a, 128, tile_h, sm_count() * per_sm);
+    if (a.R > 4) per_sm = 1;
+    const int slots = sm_count() * per_sm;
     // two planes per barrier where the registers allow it: 39.6 against 41.8 us at sigma 1 (R = 3),
     // 50.0 against 51.9 us at sigma 1.3 (R = 4), 256x256x100; no difference at R <= 2
     switch (a.R) {
-    case 1: return launch_cfg<1, 2, 4, 4, 3, 2>(a, zc, st);
-    case 2: return launch_cfg<2, 2, 4, 4, 3, 2>(a, zc, st);
-    case 3: return launch_cfg<3, 2, 4, 4, 3, 2>(a, zc, st);
-    case 4: return launch_cfg<4, 2, 4, 4, 2, 2>(a, zc, st);
-    case 5: return launch_cfg<5, 2, 8, 4, 1>(a, zc, st);
-    case 6: return launch_cfg<6, 2, 8, 4, 1>(a, zc, st);
+    case 1: return launch_cfg<1, 2, 4, 4, 3, 2>(a, slots, st);
+    case 2: return launch_cfg<2, 2, 4, 4, 3, 2>(a, slots, st);
+    case 3: return launch_cfg<3, 2, 4, 4, 3, 2>(a, slots, st);
+    case 4: return launch_cfg<4, 2, 4, 4, 2, 2>(a, slots, st);
+    case 5: return launch_cfg<5, 2, 8, 4, 1, 1, 1, 1>(a, slots, st);
+    case 6: return launch_cfg<6, 2, 8, 4, 1, 1, 1, 1>(a, slots, st);
     default: return 0;
     }
 }
