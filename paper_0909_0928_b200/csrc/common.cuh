@@ -25,7 +25,8 @@ struct Control {
     unsigned int level_iter;   // iterations executed on the current level
     int stop_force;            // set when the stopping rule fires; force kernels then skip
     int stop_smooth;           // set by the first skipped force kernel; smoothing then skips
-    int pad0[11];
+    unsigned int nblocks;      // deferred metrics: block partials the last force kernel wrote for this pair
+    int pad0[10];
     int lvalid[LHIST];         // l_n defined (sum|u| > 0)
     double lhist[LHIST];       // ring of relative norms l_n of this level
     int iters_done[8];         // per level, copied from level_iter when the level ends
@@ -45,6 +46,7 @@ struct MetricSink {
     int stride;         // capacity of one partial row (>= number of blocks per pair)
     int driver;         // 1 inside demons_register: rows advance, the stopping rule runs, stop flags are honoured
     double eps;         // stopping rule threshold (<= 0: off)
+    int defer;          // 1: force blocks only store their partials; k_metrics_final sums and publishes them
 };
 
 __device__ __forceinline__ float lerpf(float a, float b, float t) { return fmaf(t, b - a, a); }
@@ -246,6 +248,59 @@ __device__ __forceinline__ double warp_max(double v) {
     return v;
 }
 
+// Fixed-order sum (max for the last NMAX) of the `nblocks` block partials of NV quantities; the totals end up in v of
+// thread 0.  Must be called by every thread of the block.
+template <int NV, int NMAX = 0>
+__device__ __forceinline__ void final_sum(double (&v)[NV], const double* partials, int stride, unsigned int nblocks) {
+    __shared__ double fs[NV][32];
+    const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+    const int nthreads = blockDim.x * blockDim.y * blockDim.z;
+    const int lane = tid & 31, wid = tid >> 5, nwarps = (nthreads + 31) >> 5;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+        const bool is_max = i >= NV - NMAX;
+        double r = is_max ? -1.0e300 : 0.0;
+        const volatile double* p = partials + (size_t)i * stride;
+        for (unsigned int b = tid; b < nblocks; b += nthreads) r = is_max ? fmax(r, p[b]) : r + p[b];
+        r = is_max ? warp_max(r) : warp_sum(r);
+        if (lane == 0) fs[i][wid] = r;
+    }
+    __syncthreads();
+    if (wid == 0) {
+#pragma unroll
+        for (int i = 0; i < NV; ++i) {
+            const bool is_max = i >= NV - NMAX;
+            double q = lane < nwarps ? fs[i][lane] : (is_max ? -1.0e300 : 0.0);
+            q = is_max ? warp_max(q) : warp_sum(q);
+            v[i] = q;
+        }
+    }
+}
+
+// Block-wide reduction of NV doubles and publication of the block partial, nothing else: the deferred form, summed
+// later by k_metrics_final (no fence, no ticket: the kernel boundary orders the partials).
+template <int NV>
+__device__ __forceinline__ void block_reduce_store(double (&v)[NV], double* partials, int stride, unsigned int bid) {
+    __shared__ double sm[NV][32];
+    const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+    const int nthreads = blockDim.x * blockDim.y * blockDim.z;
+    const int lane = tid & 31, wid = tid >> 5, nwarps = (nthreads + 31) >> 5;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+        const double r = warp_sum(v[i]);
+        if (lane == 0) sm[i][wid] = r;
+    }
+    __syncthreads();
+    if (wid == 0) {
+#pragma unroll
+        for (int i = 0; i < NV; ++i) {
+            double r = lane < nwarps ? sm[i][lane] : 0.0;
+            r = warp_sum(r);
+            if (lane == 0) partials[(size_t)i * stride + bid] = r;
+        }
+    }
+}
+
 // Block-wide reduction of NV doubles (sum; the last NMAX of them by max), publication of the
 // block partial, and the fixed-order final reduction by the last block to arrive (of the `nblocks` that
 // share this ticket; `bid` = this block's index among them).  Returns true in thread 0 of the last block,
@@ -280,22 +335,7 @@ __device__ __forceinline__ bool block_reduce_publish(double (&v)[NV], double* pa
     __syncthreads();
     if (!s_last) return false;
     __threadfence();
-#pragma unroll
-    for (int i = 0; i < NV; ++i) {
-        const bool is_max = i >= NV - NMAX;
-        double r = is_max ? -1.0e300 : 0.0;
-        const volatile double* p = partials + (size_t)i * stride;
-        for (unsigned int b = tid; b < nblocks; b += nthreads) r = is_max ? fmax(r, p[b]) : r + p[b];
-        r = is_max ? warp_max(r) : warp_sum(r);
-        __syncthreads();  // sm[][] reuse
-        if (lane == 0) sm[i][wid] = r;
-        __syncthreads();
-        if (wid == 0) {
-            double q = lane < nwarps ? sm[i][lane] : (is_max ? -1.0e300 : 0.0);
-            q = is_max ? warp_max(q) : warp_sum(q);
-            v[i] = q;
-        }
-    }
+    final_sum<NV, NMAX>(v, partials, stride, nblocks);
     if (tid == 0) *ticket = 0u;
     return tid == 0;
 }

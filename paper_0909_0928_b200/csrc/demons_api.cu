@@ -87,6 +87,9 @@ struct demons_ctx {
     double prof_ms[4] = {0, 0, 0, 0};
     long long prof_n[4] = {0, 0, 0, 0};
     std::vector<GraphEntry> graphs;
+    // side branch of an iteration: the metric finalisation runs beside the smoothing kernel (fork / join by events)
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     cudaArray_t tex_array = nullptr;
     cudaTextureObject_t tex = 0;
     Dims tex_dims{0, 0, 0};
@@ -363,6 +366,7 @@ int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb,
     fa.Sw = ic ? reinterpret_cast<float*>(c->ws + p.Sw) + (size_t)lb.b0 * N : nullptr;
     fa.sink = make_sink(c, p, lb.b0, reinterpret_cast<double*>(c->ws + p.stats) + (size_t)lb.b0 * DEMONS_MAX_STATS_ROWS * 3,
                         (size_t)DEMONS_MAX_STATS_ROWS * 3, true, eps);
+    fa.sink.defer = 1;  // the force blocks store partials; k_metrics_final (below) sums and publishes them
     fa.texM = c->opt_texture ? c->tex : 0;
     fa.l2_ptr = win.ptr;
     fa.l2_bytes = win.bytes;
@@ -379,13 +383,26 @@ int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb,
     } else {
         prof_pair(c, PROF_FORCE, e0, e1);
     }
+    // fork: statistics row and stopping rule of this iteration, beside the smoothing kernel (which reads neither)
+    if (!c->side) {
+        CUDA_TRY(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
+        CUDA_TRY(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+        CUDA_TRY(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+    }
+    CUDA_TRY(cudaEventRecord(c->ev_fork, st));
+    CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+    if (launch_metrics_final(fa.sink, lb.nb, c->side) < 0)
+        return fail(DEMONS_E_CUDA, "metrics launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    *launches += 1;
+    CUDA_TRY(cudaEventRecord(c->ev_join, c->side));
     SmoothArgs sa{};
     sa.d = lb.d;
     sa.tmp = reinterpret_cast<float*>(c->ws + p.smooth_tmp) + (size_t)lb.b0 * N;
     sa.ncomp = 3 * lb.nb;
     sa.comps_per_pair = 3;
     sa.R = gaussian_taps(c->sigma, sa.w);
-    sa.ctl = reinterpret_cast<Control*>(c->ws + p.control) + lb.b0;
+    // the smoothing kernels test the pair's stop flag only when the rule can fire
+    sa.ctl = eps > 0.0 ? reinterpret_cast<Control*>(c->ws + p.control) + lb.b0 : nullptr;
     sa.force_generic = c->opt_generic_smooth;
     sa.in = fa.u_out;
     sa.out = lb.u;
@@ -399,6 +416,7 @@ int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb,
         if (k < 0) return fail(DEMONS_E_CUDA, "smooth launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         *launches += k;
     }
+    CUDA_TRY(cudaStreamWaitEvent(st, c->ev_join, 0));  // join: the next force kernel reads the stop flag
     prof_pair(c, PROF_SMOOTH, e1, prof_event(c, st, true));
     return DEMONS_OK;
 }
@@ -647,6 +665,9 @@ void demons_destroy(demons_ctx* c) {
         cudaGetLastError();
     }
     for (auto& g : c->graphs) cudaGraphExecDestroy(g.exec);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
+    if (c->side) cudaStreamDestroy(c->side);
     release_texture(c);
     prof_clear(c);
     delete c;

@@ -41,6 +41,10 @@ struct ForceArgs {
 // S1-S4 (+S6).  Returns the number of kernels launched, or -1 with cudaGetLastError() set.
 int launch_warp_force(const ForceArgs& a, cudaStream_t stream);
 
+// Deferred metrics (sink.defer = 1 in the ForceArgs of the pass before): sums the block partials of every pair of the
+// launch and publishes them (row, stopping rule).  One launch, nb blocks.
+int launch_metrics_final(const MetricSink& sink, int nb, cudaStream_t stream);
+
 // Variant 1, once per level (and per standalone demons_warp_force call): out <- |grad I|^2, [nb][N], which
 // launch_warp_force then reads instead of stencilling M (Eq.(2) uses only the magnitude of grad M0).
 // Planes [z0, z0 + zn) of the volume only (zn < 0: all of them).

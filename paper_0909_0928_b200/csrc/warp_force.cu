@@ -26,7 +26,8 @@ constexpr int BX = 32;  // threads along x
 constexpr int BY = 8;   // threads along y (the lane-consecutive kernels may be launched with 4..8 rows)
 
 __device__ __forceinline__ bool skip_pass(const MetricSink& s, unsigned b) {
-    if (s.driver && *reinterpret_cast<volatile int*>(&s.ctl[b].stop_force) != 0) {
+    // eps <= 0: the rule is off and the flag can never be set -- no load (an L2 round trip before the first useful one)
+    if (s.driver && s.eps > 0.0 && *reinterpret_cast<volatile int*>(&s.ctl[b].stop_force) != 0) {
         s.ctl[b].stop_smooth = 1;
         return true;
     }
@@ -61,9 +62,28 @@ __device__ __forceinline__ void reduce_metrics(double (&acc)[3], const MetricSin
                                                unsigned chunks) {
     if (s.out == nullptr) return;
     const unsigned bid = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * chunk);
-    if (block_reduce_publish<3>(acc, s.partials + (size_t)b * 5 * s.stride, s.stride, &s.ctl[b].ticket, bid,
-                                gridDim.x * gridDim.y * chunks))
+    const unsigned nblocks = gridDim.x * gridDim.y * chunks;
+    if (s.defer) {
+        // inside a registration: the fence, the ticket and the last block's final sum were 4.8 of the 47 us of the
+        // fused pass at 256x256x100 (the tail of the kernel); k_metrics_final does them beside the smoothing kernel
+        block_reduce_store<3>(acc, s.partials + (size_t)b * 5 * s.stride, s.stride, bid);
+        if (bid == 0 && threadIdx.x == 0 && threadIdx.y == 0) s.ctl[b].nblocks = nblocks;
+        return;
+    }
+    if (block_reduce_publish<3>(acc, s.partials + (size_t)b * 5 * s.stride, s.stride, &s.ctl[b].ticket, bid, nblocks))
         publish_metrics(acc, s, b);
+}
+
+// Deferred metrics (MetricSink::defer): one block per pair sums the block partials of the force kernel that has
+// just finished, in a fixed order, writes the statistics row and applies the stopping rule.  Runs on a side branch
+// of the iteration, beside the smoothing kernel; the next force kernel waits for both.
+__global__ void __launch_bounds__(256) k_metrics_final(const MetricSink s) {
+    const unsigned b = blockIdx.x;
+    // the force pass of this iteration was skipped (the rule fired earlier): nothing was written
+    if (s.driver && *reinterpret_cast<volatile int*>(&s.ctl[b].stop_smooth) != 0) return;
+    double v[3];
+    final_sum<3>(v, s.partials + (size_t)b * 5 * s.stride, s.stride, s.ctl[b].nblocks);
+    if (threadIdx.x == 0) publish_metrics(v, s, b);
 }
 
 // Eq.(1): F = q(d, d^2 + |g|^2) g, with alpha^2 d^2 for Eq.(5).  Returns the scalar factor.
@@ -932,6 +952,11 @@ int launch_negate(const float* in, float* out, size_t n, cudaStream_t st) {
     size_t blocks = (n + 255) / 256;
     if (blocks > (size_t)sm_count() * 16) blocks = (size_t)sm_count() * 16;
     k_negate<<<(unsigned)(blocks < 1 ? 1 : blocks), 256, 0, st>>>(in, out, n);
+    return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
+}
+
+int launch_metrics_final(const MetricSink& sink, int nb, cudaStream_t st) {
+    k_metrics_final<<<nb, 256, 0, st>>>(sink);
     return cudaPeekAtLastError() == cudaSuccess ? 1 : -1;
 }
 
