@@ -427,7 +427,7 @@ def main():
     prof = B.demons_get_profile(eng.ctx)
     launches_per_iter = (B.demons_launch_count(eng.ctx) - l0) / sum(ITERS)
     B.demons_set_option(eng.ctx, "profile", 0)
-    smooth_launches = launches_per_iter - 1
+    smooth_launches = launches_per_iter - 2  # per iteration: the force kernel, k_metrics_final (side branch), the smoother
     bytes_per_voxel = {"force": 32.0, "smooth": 24.0 if smooth_launches <= 1 else 72.0}
     kernel_names = {"force": "k_force_fixed_lc<0,4> (fused warp+gradient+force+update+metrics, lane-consecutive cells)",
                     "smooth": "k_smooth_tma<3> (TMA-fed single pass, 3 components)" if smooth_launches <= 1
