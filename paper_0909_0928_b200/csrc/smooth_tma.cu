@@ -388,14 +388,16 @@ __global__ void __launch_bounds__(32 * (RG + 1), MINB)
     }
 }
 
-// Planes per CTA: the number of z chunks that minimises  waves x (planes per chunk + 2R warm-up).
+// Planes per CTA: the number of z chunks that minimises  waves x (planes per chunk + 2R warm-up + start-up).  Small
+// volumes end up with very short chunks (2-3 planes behind 2R warm-up planes): the machine is mostly empty there and
+// the length of the march counts, not the number of CTAs (64x64x25: 9.4 -> 9.2 us per iteration with chunks of 2
+// instead of 7 planes; start-up and drain dominate at that size).
 int pick_zc(const SmoothArgs& a, int tile_w, int tile_h, int slots) {
     const long long tiles = (long long)((a.d.nx + tile_w - 1) / tile_w) * ((a.d.ny + tile_h - 1) / tile_h) * a.ncomp;
     int best_zc = a.d.nz;
     double best = 1e300;
     for (int chunks = 1; chunks <= a.d.nz; ++chunks) {
         const int zc = (a.d.nz + chunks - 1) / chunks;
-        if (chunks > 1 && zc < 2 * a.R) break;
         const long long ctas = tiles * ((a.d.nz + zc - 1) / zc);
         const double waves = (double)((ctas + slots - 1) / slots);
         const double cost = waves * (zc + 2 * a.R + 2);
