@@ -1,11 +1,12 @@
 """BASELINE.json config 5: bandwidth sweep of the per-iteration kernels through the C ABI.
 
     python -m paper_0909_0928_b200.sweep [--sizes 128x128x64,256x256x100,...] [--reps 20]
-                                         [--kernels force,smooth,pyramid,texture] [--json out.json]
+                                         [--kernels force,iteration,smooth,pyramid,texture] [--json out.json]
 
 For every size: the fused warp+force+update entry point for all six variants, the Gaussian
 smoothing at sigma 1.0 and 2.0 (3 components), restrict and prolong.  Inputs are the seeded blob
-phantom and a random smooth field with max |u| = 8 voxels (phantoms.sweep_inputs).  Reported per
+phantom and a random smooth field with max |u| = 8 voxels (phantoms.sweep_inputs).  `iteration[...]` rows time one
+whole [force ; smooth] iteration inside a registration (40 iterations, one level, sigma 1).  Reported per
 kernel: median over `reps` samples of 10 back-to-back launches (CUDA events) after 3 warm-ups, effective GB/s = algorithmic
 bytes (DESIGN.md byte table) / time, and % of the measured HBM peak.  The same command with
 --reps 1 --warmups 1 --inner 1 (every entry point launched twice) is what the ncu captures under profiles/ run.  S and M are separate allocations here, so the L2
@@ -107,6 +108,25 @@ def run(sizes, kernels, reps, device="cuda:0"):
             rows[-1]["mean_abs_err_vs_software_voxel"] = float(err.mean())
             rows[-1]["frac_outside_1e-4"] = float((err > 1e-4).float().mean())
             eng.close()
+        if "iteration" in kernels:
+            # one whole iteration INSIDE a registration ([force ; smooth], sigma 1, per-level CUDA graph): what the
+            # standalone rows cannot show -- there the metric totals are finalised by the force kernel's last block (a
+            # fence, a ticket and a serial sum at the tail of the kernel), here by k_metrics_final beside the smoother
+            its = 40
+            for variant in range(6):
+                eng = B.Demons(dims, variant=variant, alpha=0.4 if variant == 4 else 1.0, sigma=1.0, device=device)
+                ic = variant == 5
+                out.copy_(du)  # the registrations continue from the sweep's field (max |u| = 8), one after another
+                if ic:
+                    outb.copy_(dub)
+                torch.cuda.synchronize()
+                ms = median_ms(torch, stream, lambda: B.demons_register(
+                    eng.ctx, dS, dM, out, outb if ic else None, [its], 0.0, None, None, stream), max(3, reps // 4), inner=1) / its
+                # force bytes inside a registration: variant 1 without the per-level |grad M|^2 pass; variant 5 starts
+                # from the caller's fields here, i.e. the two-field form (96 B/voxel, both fields smoothed: 48)
+                fb = {0: 32.0, 1: 36.0, 2: 52.0, 3: 52.0, 4: 52.0, 5: 96.0}[variant]
+                add(f"iteration[{VARIANT_NAMES[variant]}]", ms, (fb + (48.0 if ic else 24.0)) * N)
+                eng.close()
         eng = B.Demons(dims, variant=0, device=device)
         if "smooth" in kernels:
             for sigma in (1.0, 2.0):
@@ -127,7 +147,7 @@ def run(sizes, kernels, reps, device="cuda:0"):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--sizes", default="128x128x64,256x256x100,512x512x160,512x512x256")
-    ap.add_argument("--kernels", default="force,smooth,pyramid,texture")
+    ap.add_argument("--kernels", default="force,iteration,smooth,pyramid,texture")
     ap.add_argument("--reps", type=int, default=20)
     ap.add_argument("--json", default=None)
     ap.add_argument("--warmups", type=int, default=3)
