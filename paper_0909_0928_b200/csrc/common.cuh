@@ -25,8 +25,7 @@ struct Control {
     unsigned int level_iter;   // iterations executed on the current level
     int stop_force;            // set when the stopping rule fires; force kernels then skip
     int stop_smooth;           // set by the first skipped force kernel; smoothing then skips
-    unsigned int nblocks;      // deferred metrics: block partials the last force kernel wrote for this pair
-    int pad0[10];
+    int pad0[11];
     int lvalid[LHIST];         // l_n defined (sum|u| > 0)
     double lhist[LHIST];       // ring of relative norms l_n of this level
     int iters_done[8];         // per level, copied from level_iter when the level ends
@@ -47,6 +46,7 @@ struct MetricSink {
     int driver;         // 1 inside demons_register: rows advance, the stopping rule runs, stop flags are honoured
     double eps;         // stopping rule threshold (<= 0: off)
     int defer;          // 1: force blocks only store their partials; k_metrics_final sums and publishes them
+    unsigned nblocks;   // k_metrics_final only: block partials per pair written by the force kernel before it
 };
 
 __device__ __forceinline__ float lerpf(float a, float b, float t) { return fmaf(t, b - a, a); }

@@ -373,6 +373,8 @@ int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb,
     fa.l2_ratio = win.ratio;
     cudaEvent_t e0 = prof_event(c, st, true);
     fa.ev_mid = c->variant >= DEMONS_ACTIVE ? prof_event(c, st, false) : nullptr;
+    int metric_blocks = 0;
+    fa.metric_blocks = &metric_blocks;
     int k = launch_warp_force(fa, st);
     if (k < 0) return fail(DEMONS_E_CUDA, "warp_force launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     *launches += k;
@@ -391,6 +393,7 @@ int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb,
     }
     CUDA_TRY(cudaEventRecord(c->ev_fork, st));
     CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+    fa.sink.nblocks = (unsigned)metric_blocks;
     if (launch_metrics_final(fa.sink, lb.nb, c->side) < 0)
         return fail(DEMONS_E_CUDA, "metrics launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     *launches += 1;

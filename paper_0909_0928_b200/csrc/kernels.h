@@ -28,6 +28,7 @@ struct ForceArgs {
     MetricSink sink;
     cudaTextureObject_t texM;  // 0 = software trilinear (default); nb must be 1 otherwise
     cudaEvent_t ev_mid;        // nullable: recorded between the warp and the force kernel (profiling)
+    int* metric_blocks;        // nullable out: block partials per pair the pass wrote (sink.nblocks of k_metrics_final)
     // z-slab form (one rank of a z-slab decomposition): d is the local slab (fields, warped images), which starts at
     // plane zoff of the images; S and M are whole volumes of gnz planes; planes [mz0, mz1) of the slab count in the
     // metrics.  nb must be 1, texM 0.
@@ -42,7 +43,7 @@ struct ForceArgs {
 int launch_warp_force(const ForceArgs& a, cudaStream_t stream);
 
 // Deferred metrics (sink.defer = 1 in the ForceArgs of the pass before): sums the block partials of every pair of the
-// launch and publishes them (row, stopping rule).  One launch, nb blocks.
+// launch (sink.nblocks of them per pair) and publishes them (row, stopping rule).  One launch, nb blocks.
 int launch_metrics_final(const MetricSink& sink, int nb, cudaStream_t stream);
 
 // Variant 1, once per level (and per standalone demons_warp_force call): out <- |grad I|^2, [nb][N], which

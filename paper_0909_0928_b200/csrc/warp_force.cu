@@ -36,16 +36,15 @@ __device__ __forceinline__ bool skip_pass(const MetricSink& s, unsigned b) {
 
 // Thread 0 of the last block of pair b: write {SSD, sum|F|, sum|u|}, advance the row, apply the stopping
 // rule  l_n = sum|F| / sum|u|;  stop after the first n >= 10 with |l_n - l_{n-10}| <= eps.
-__device__ __forceinline__ void publish_metrics(const double (&v)[3], const MetricSink& s, unsigned b) {
+__device__ __forceinline__ void publish_metrics_at(const double (&v)[3], const MetricSink& s, unsigned b, unsigned row,
+                                                   unsigned n) {
     Control& c = s.ctl[b];
-    const unsigned int row = s.driver ? c.row_counter : 0u;
     double* o = s.out + (size_t)b * s.out_stride + 3 * (size_t)row;
     o[0] = v[0];
     o[1] = v[1];
     o[2] = v[2];
     if (s.driver) {
         c.row_counter = row + 1u;
-        const unsigned int n = c.level_iter;
         const int valid = v[2] > 0.0;
         const double l = valid ? v[1] / v[2] : 0.0;
         c.lhist[n & (LHIST - 1)] = l;
@@ -55,6 +54,9 @@ __device__ __forceinline__ void publish_metrics(const double (&v)[3], const Metr
             c.stop_force = 1;
         c.level_iter = n + 1u;
     }
+}
+__device__ __forceinline__ void publish_metrics(const double (&v)[3], const MetricSink& s, unsigned b) {
+    publish_metrics_at(v, s, b, s.driver ? s.ctl[b].row_counter : 0u, s.driver ? s.ctl[b].level_iter : 0u);
 }
 
 // Block-wide reduction of the three metrics of pair b and their publication by the last block of the pair.
@@ -67,7 +69,6 @@ __device__ __forceinline__ void reduce_metrics(double (&acc)[3], const MetricSin
         // inside a registration: the fence, the ticket and the last block's final sum were 4.8 of the 47 us of the
         // fused pass at 256x256x100 (the tail of the kernel); k_metrics_final does them beside the smoothing kernel
         block_reduce_store<3>(acc, s.partials + (size_t)b * 5 * s.stride, s.stride, bid);
-        if (bid == 0 && threadIdx.x == 0 && threadIdx.y == 0) s.ctl[b].nblocks = nblocks;
         return;
     }
     if (block_reduce_publish<3>(acc, s.partials + (size_t)b * 5 * s.stride, s.stride, &s.ctl[b].ticket, bid, nblocks))
@@ -80,10 +81,16 @@ __device__ __forceinline__ void reduce_metrics(double (&acc)[3], const MetricSin
 __global__ void __launch_bounds__(256) k_metrics_final(const MetricSink s) {
     const unsigned b = blockIdx.x;
     // the force pass of this iteration was skipped (the rule fired earlier): nothing was written
-    if (s.driver && *reinterpret_cast<volatile int*>(&s.ctl[b].stop_smooth) != 0) return;
+    if (s.driver && s.eps > 0.0 && *reinterpret_cast<volatile int*>(&s.ctl[b].stop_smooth) != 0) return;
+    // the cursors are read before the sum, not behind its barriers: one L2 round trip for everything this block loads
+    unsigned row = 0u, n = 0u;
+    if (threadIdx.x == 0 && s.driver) {
+        row = *reinterpret_cast<volatile unsigned*>(&s.ctl[b].row_counter);
+        n = *reinterpret_cast<volatile unsigned*>(&s.ctl[b].level_iter);
+    }
     double v[3];
-    final_sum<3>(v, s.partials + (size_t)b * 5 * s.stride, s.stride, s.ctl[b].nblocks);
-    if (threadIdx.x == 0) publish_metrics(v, s, b);
+    final_sum<3>(v, s.partials + (size_t)b * 5 * s.stride, s.stride, s.nblocks);
+    if (threadIdx.x == 0) publish_metrics_at(v, s, b, row, n);
 }
 
 // Eq.(1): F = q(d, d^2 + |g|^2) g, with alpha^2 d^2 for Eq.(5).  Returns the scalar factor.
@@ -757,6 +764,7 @@ int launch_lc(const ForceArgs& a, bool vec4, cudaStream_t st) {
         p.zper = sh.zper;
         p.chunks = (a.d.nz + sh.zper - 1) / sh.zper;
         const dim3 grid(tiles_x, (a.d.ny + sh.by - 1) / sh.by, p.chunks * a.nb);
+        if (a.metric_blocks && a.variant <= 1) *a.metric_blocks = (int)(grid.x * grid.y) * p.chunks;
         // The gathered image is re-read by every iteration and is the one stream whose misses sit on the
         // critical path (the gathers): an access-policy window asks L2 to keep it (persisting) while the
         // field streams through.  At 256x256x100 the fused pass goes from 54 to 49.7 us.
@@ -805,6 +813,7 @@ int launch_lc(const ForceArgs& a, bool vec4, cudaStream_t st) {
         const Shape sh = pick_shape(kernel, tx, a.d.ny, a.d.nz, a.nb, blocks_cap(a), BY, BY);
         p.zper = sh.zper;
         p.chunks = (a.d.nz + sh.zper - 1) / sh.zper;
+        if (a.metric_blocks) *a.metric_blocks = tx * ((a.d.ny + BY - 1) / BY) * p.chunks;
         kernel<<<dim3(tx, (a.d.ny + BY - 1) / BY, p.chunks * a.nb), dim3(BX, BY), 0, st>>>(p);
     };
     if (a.slab) {
@@ -860,6 +869,7 @@ int launch_generic(const ForceArgs& a, cudaStream_t st) {
     p.zper = ZPER;
     p.chunks = (a.d.nz + ZPER - 1) / ZPER;
     const dim3 block(BX, BY), grid((a.d.nx + BX - 1) / BX, (a.d.ny + BY - 1) / BY, p.chunks * a.nb);
+    if (a.metric_blocks) *a.metric_blocks = (int)(grid.x * grid.y) * p.chunks;
     switch (a.variant) {
     case 0: k_force_fixed<0><<<grid, block, 0, st>>>(p); return 1;
     case 1: k_force_fixed<1><<<grid, block, 0, st>>>(p); return 1;
