@@ -342,6 +342,15 @@ struct LevelBuffers {
     int one_field;
 };
 
+// The side stream of the metric finalisation and its fork / join events; created outside any stream capture.
+int ensure_side(demons_ctx* c) {
+    if (c->side) return DEMONS_OK;
+    CUDA_TRY(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
+    CUDA_TRY(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+    CUDA_TRY(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+    return DEMONS_OK;
+}
+
 // One iteration of a group of pairs: [warp_force ; smooth the total field] (reading C2).
 int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb, const L2Window& win, double eps,
                       cudaStream_t st, int* launches) {
@@ -386,11 +395,6 @@ int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb,
         prof_pair(c, PROF_FORCE, e0, e1);
     }
     // fork: statistics row and stopping rule of this iteration, beside the smoothing kernel (which reads neither)
-    if (!c->side) {
-        CUDA_TRY(cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking));
-        CUDA_TRY(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
-        CUDA_TRY(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
-    }
     CUDA_TRY(cudaEventRecord(c->ev_fork, st));
     CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
     fa.sink.nblocks = (unsigned)metric_blocks;
@@ -516,6 +520,7 @@ int register_impl(demons_ctx* c, const float* dS, const float* dM, float* du, fl
     // iterated on and u_b is written once on exit; bit-identical to iterating on both fields
     const int one_field = ic && zero_start && c->opt_ic_one_field ? 1 : 0;
     prof_clear(c);
+    if (const int rs = ensure_side(c); rs != DEMONS_OK) return rs;
     CUDA_TRY(cudaMemsetAsync(ctl, 0, (size_t)nb * sizeof(Control), st));
     if (total_iters > 0)
         CUDA_TRY(cudaMemsetAsync(c->ws + p.stats, 0,

@@ -20,6 +20,7 @@ import argparse
 import json
 import os
 import sys
+import time
 
 import numpy as np
 
@@ -40,13 +41,14 @@ def hbm_peak():
         return 6650.0, "fallback"
 
 
-WARMUPS, INNER = 3, 10
+WARMUPS, INNER, PAUSE_S = 3, 10, 0.3
 
 
 def median_ms(torch, stream, fn, reps, inner=None):
     """Median over `reps` samples of (CUDA-event time of `inner` back-to-back launches) / inner: the
     queue stays full, so the host's launch latency is not in the number."""
     inner = INNER if inner is None else inner
+    time.sleep(PAUSE_S)  # every row starts from the same power state (a long sweep runs into the board's power cap)
     for _ in range(WARMUPS):
         fn()
     torch.cuda.synchronize()
@@ -108,6 +110,20 @@ def run(sizes, kernels, reps, device="cuda:0"):
             rows[-1]["mean_abs_err_vs_software_voxel"] = float(err.mean())
             rows[-1]["frac_outside_1e-4"] = float((err > 1e-4).float().mean())
             eng.close()
+        eng = B.Demons(dims, variant=0, device=device)
+        if "smooth" in kernels:
+            for sigma in (1.0, 2.0):
+                ms = median_ms(torch, stream, lambda: B.demons_smooth(eng.ctx, dims, du, out, 3, sigma, stream), reps)
+                add(f"smooth[sigma={sigma}]", ms, 24.0 * N)
+        if "pyramid" in kernels:
+            cd = B.demons_level_dims(eng.ctx, 1)
+            coarse = torch.empty((cd[2], cd[1], cd[0]), dtype=torch.float32, device=device)
+            uc = torch.randn((3, cd[2], cd[1], cd[0]), dtype=torch.float32, device=device)
+            ms = median_ms(torch, stream, lambda: B.demons_restrict(eng.ctx, dims, dS, coarse, stream), reps)
+            add("restrict", ms, 4.5 * N)
+            ms = median_ms(torch, stream, lambda: B.demons_prolong(eng.ctx, cd, uc, dims, out, stream), reps)
+            add("prolong", ms, 13.5 * N)
+        eng.close()
         if "iteration" in kernels:
             # one whole iteration INSIDE a registration ([force ; smooth], sigma 1, per-level CUDA graph): what the
             # standalone rows cannot show -- there the metric totals are finalised by the force kernel's last block (a
@@ -127,20 +143,6 @@ def run(sizes, kernels, reps, device="cuda:0"):
                 fb = {0: 32.0, 1: 36.0, 2: 52.0, 3: 52.0, 4: 52.0, 5: 96.0}[variant]
                 add(f"iteration[{VARIANT_NAMES[variant]}]", ms, (fb + (48.0 if ic else 24.0)) * N)
                 eng.close()
-        eng = B.Demons(dims, variant=0, device=device)
-        if "smooth" in kernels:
-            for sigma in (1.0, 2.0):
-                ms = median_ms(torch, stream, lambda: B.demons_smooth(eng.ctx, dims, du, out, 3, sigma, stream), reps)
-                add(f"smooth[sigma={sigma}]", ms, 24.0 * N)
-        if "pyramid" in kernels:
-            cd = B.demons_level_dims(eng.ctx, 1)
-            coarse = torch.empty((cd[2], cd[1], cd[0]), dtype=torch.float32, device=device)
-            uc = torch.randn((3, cd[2], cd[1], cd[0]), dtype=torch.float32, device=device)
-            ms = median_ms(torch, stream, lambda: B.demons_restrict(eng.ctx, dims, dS, coarse, stream), reps)
-            add("restrict", ms, 4.5 * N)
-            ms = median_ms(torch, stream, lambda: B.demons_prolong(eng.ctx, cd, uc, dims, out, stream), reps)
-            add("prolong", ms, 13.5 * N)
-        eng.close()
     return rows, peak, peak_kind
 
 

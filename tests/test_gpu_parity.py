@@ -139,7 +139,7 @@ SMOOTH_DIMS = [(64, 64, 32), (136, 44, 21), (37, 29, 19), (8, 5, 3), (4, 2, 1), 
 
 
 @pytest.mark.parametrize("dims", SMOOTH_DIMS)
-@pytest.mark.parametrize("sigma,ncomp", [(1.0, 3), (2.0, 3), (0.7, 1), (0.3, 2), (3.5, 3), (1.0, 6)])
+@pytest.mark.parametrize("sigma,ncomp", [(1.0, 3), (2.0, 3), (0.7, 1), (0.3, 2), (3.5, 3), (1.0, 6), (1.3, 2), (1.6, 3), (2.0, 6)])
 def test_smooth_matches_oracle(torch_cuda, B, oracle, dims, sigma, ncomp):
     torch = torch_cuda
     rng = np.random.default_rng(17)
@@ -326,13 +326,13 @@ def test_alpha_one_equals_double_force_on_gpu(torch_cuda, B, P):  # P8 through t
     assert np.array_equal(a["u"], b["u"])
 
 
-def run_register_batch(torch, B, variant, pairs, iters, alpha=1.0, eps=0.0, options=()):
+def run_register_batch(torch, B, variant, pairs, iters, alpha=1.0, eps=0.0, options=(), sigma=1.0):
     """demons_register_batch on a list of (S, M) pairs of one size; returns per-pair results."""
     nb = len(pairs)
     S0 = pairs[0][0]
     dims = (S0.shape[2], S0.shape[1], S0.shape[0])
     ic = variant == 5
-    eng = B.Demons(dims, variant=variant, alpha=alpha, levels=len(iters), nbatch=nb)
+    eng = B.Demons(dims, variant=variant, alpha=alpha, sigma=sigma, levels=len(iters), nbatch=nb)
     for name, value in options:
         B.demons_set_option(eng.ctx, name, value)
     dS = dev(torch, np.stack([p[0] for p in pairs]))
@@ -395,6 +395,28 @@ def test_register_batch_groups_and_early_stop(torch_cuda, B, P, oracle):
         assert np.all(stats[k, n:] == 0.0)
         stops.append(n)
     assert len(set(stops)) > 1 and min(stops) < 60, stops
+
+
+@pytest.mark.parametrize("variant", [0, 3])
+def test_register_batch_sigma2_shares_and_early_stop(torch_cuda, B, P, variant):
+    """sigma = 2 (R = 6): the smoothing kernel splits the columns of ALL pairs into equal shares of one wave, so a CTA's
+    run of planes crosses from one component / pair into the next, and the stop flag is tested per segment.  The batch
+    still equals the single registrations bit for bit, with eps > 0 stopping every pair on its own iteration."""
+    torch = torch_cuda
+    dims = (40, 36, 18)
+    pairs = [P.config1_pair(dims=dims, seed=70 + k, noise_sd=0.0, max_norm=1.0 + 0.4 * k)[:2] for k in range(5)]
+    eps = 3e-3
+    alpha = ALPHA.get(variant, 1.0)
+    u, _, stats, done, _ = run_register_batch(torch, B, variant, pairs, [50], alpha=alpha, eps=eps, options=(("zero_start", 1),),
+                                              sigma=2.0)
+    stops = []
+    for k, (S, M) in enumerate(pairs):
+        one = run_register(torch, B, variant, S, M, [50], alpha=alpha, sigma=2.0, eps=eps)
+        assert np.array_equal(u[k], one["u"]), f"pair {k}"
+        assert done[k].tolist() == one["iters_done"]
+        np.testing.assert_allclose(stats[k], one["stats"], rtol=1e-12, atol=0)
+        stops.append(one["iters_done"][0])
+    assert min(stops) >= 10, stops
 
 
 def test_inverse_consistent_one_field_is_bit_identical(torch_cuda, B, P, oracle):
