@@ -158,6 +158,21 @@ int demons_register_host(demons_ctx* ctx, const float* h_static, const float* h_
                          float* h_u_back, int levels, const int* h_iters_per_level, double eps,
                          double* h_stats, int* h_iters_done, void* stream);
 
+/* A QUEUE of n registrations of equally sized pairs from host buffers (the paper's use case: many registrations per
+ * patient course), run one after another on `stream` exactly as demons_register_host runs each of them,
+ * with two staging slots in the workspace: the upload of pair k + 1 and the download of field k - 1 ride on two internal
+ * streams beside registration k, so that the PCIe transfers (8 B/voxel up, 12 B/voxel down per registration) cost no
+ * GPU time except for the first upload and the last download.  h_static, h_moving, h_u (and h_u_back, variant 5; NULL
+ * otherwise) are arrays of n HOST pointers; the same buffer may appear several times (downloads are ordered).  Pinned
+ * host memory is what makes the overlap possible; pageable memory works and serialises.  h_stats (nullable)
+ * [n][sum iters][3], h_iters_done (nullable) [n][levels].  Results are bit-identical to n demons_register_host calls.
+ * Needs a workspace of demons_workspace_bytes_queue(ctx, levels) (the single-registration workspace plus the second
+ * staging slot); synchronises before returning. */
+size_t demons_workspace_bytes_queue(const demons_ctx* ctx, int levels);
+int demons_register_host_queue(demons_ctx* ctx, int n, const float* const* h_static, const float* const* h_moving,
+                               float* const* h_u, float* const* h_u_back, int levels, const int* h_iters_per_level,
+                               double eps, double* h_stats, int* h_iters_done, void* stream);
+
 /* ---- per-kernel entry points (one pass each, what the parity tests and the sweep call) -------
  * All take explicit dims (nx*ny*nz must not exceed the context's finest volume).
  *

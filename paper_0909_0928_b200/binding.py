@@ -39,6 +39,9 @@ SIGNATURES = {
                                              _vp, _vp, _vp]),
     "demons_register_host": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, ctypes.c_int, _c_int3, ctypes.c_double, _vp,
                                             _vp, _vp]),
+    "demons_workspace_bytes_queue": (ctypes.c_size_t, [_vp, ctypes.c_int]),
+    "demons_register_host_queue": (ctypes.c_int, [_vp, ctypes.c_int, _vp, _vp, _vp, _vp, ctypes.c_int, _c_int3,
+                                                  ctypes.c_double, _vp, _vp, _vp]),
     "demons_warp_force": (ctypes.c_int, [_vp, _c_int3, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "demons_warp_force_slab": (ctypes.c_int, [_vp, _c_int3, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, _vp, _vp,
                                               _vp, _vp, _vp, _vp, _vp, _vp]),
@@ -181,6 +184,24 @@ def demons_register_host(ctx, h_static, h_moving, h_u, h_u_back, iters_per_level
                                       float(eps), _ptr(h_stats), _ptr(h_iters_done), _stream(stream)))
 
 
+def demons_workspace_bytes_queue(ctx, levels):
+    return int(lib().demons_workspace_bytes_queue(ctx, int(levels)))
+
+
+def demons_register_host_queue(ctx, h_static, h_moving, h_u, h_u_back, iters_per_level, eps=0.0, h_stats=None,
+                               h_iters_done=None, stream=None):
+    """h_static, h_moving, h_u (h_u_back): sequences of n host buffers (pinned torch tensors or numpy arrays)."""
+    n = len(h_static)
+    levels = len(iters_per_level)
+    it = (ctypes.c_int * levels)(*[int(i) for i in iters_per_level])
+
+    def ptrs(seq):
+        return None if seq is None else (ctypes.c_void_p * n)(*[_ptr(t) for t in seq])
+    pS, pM, pU, pUb = ptrs(h_static), ptrs(h_moving), ptrs(h_u), ptrs(h_u_back)
+    _check(lib().demons_register_host_queue(ctx, n, pS, pM, pU, pUb, levels, it, float(eps), _ptr(h_stats),
+                                            _ptr(h_iters_done), _stream(stream)))
+
+
 def demons_warp_force(ctx, dims, d_static, d_moving, d_u_in, d_u_out, d_ub_in=None, d_ub_out=None, d_metrics=None,
                       stream=None):
     _check(lib().demons_warp_force(ctx, _int3(dims), _ptr(d_static), _ptr(d_moving), _ptr(d_u_in), _ptr(d_u_out),
@@ -235,7 +256,7 @@ class Demons:
     """Owns a demons_ctx and the torch tensor backing its workspace (allocation only)."""
 
     def __init__(self, dims, spacing=(1.0, 1.0, 1.0), variant=PASSIVE, alpha=1.0, sigma=1.0, levels=1,
-                 device="cuda:0", nbatch=1):
+                 device="cuda:0", nbatch=1, queue=False):
         import torch
         self.dims = tuple(int(d) for d in dims)
         self.variant = int(variant)
@@ -244,6 +265,8 @@ class Demons:
         self.ctx = demons_create(self.dims, spacing, variant, alpha, sigma)
         self.nbatch = int(nbatch)
         nbytes = demons_workspace_bytes_batch(self.ctx, levels, nbatch)
+        if queue:  # second staging slot of demons_register_host_queue
+            nbytes = max(nbytes, demons_workspace_bytes_queue(self.ctx, levels))
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=device)
         off = (-self.workspace.data_ptr()) % 256
         self._ws_ptr = self.workspace.data_ptr() + off

@@ -90,6 +90,10 @@ struct demons_ctx {
     // side branch of an iteration: the metric finalisation runs beside the smoothing kernel (fork / join by events)
     cudaStream_t side = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    // demons_register_host_queue: copy-in and copy-out streams, per staging slot the events "images uploaded",
+    // "registration done" and "field downloaded"
+    cudaStream_t q_in = nullptr, q_out = nullptr;
+    cudaEvent_t q_up[2] = {nullptr, nullptr}, q_done[2] = {nullptr, nullptr}, q_down[2] = {nullptr, nullptr};
     cudaArray_t tex_array = nullptr;
     cudaTextureObject_t tex = 0;
     Dims tex_dims{0, 0, 0};
@@ -676,6 +680,13 @@ void demons_destroy(demons_ctx* c) {
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
     if (c->side) cudaStreamDestroy(c->side);
+    for (int k = 0; k < 2; ++k) {
+        if (c->q_up[k]) cudaEventDestroy(c->q_up[k]);
+        if (c->q_done[k]) cudaEventDestroy(c->q_done[k]);
+        if (c->q_down[k]) cudaEventDestroy(c->q_down[k]);
+    }
+    if (c->q_in) cudaStreamDestroy(c->q_in);
+    if (c->q_out) cudaStreamDestroy(c->q_out);
     release_texture(c);
     prof_clear(c);
     delete c;
@@ -789,6 +800,118 @@ int demons_register_host(demons_ctx* c, const float* h_static, const float* h_mo
         CUDA_TRY(cudaMemcpyAsync(h_stats, c->ws + p.stats, (size_t)total_iters * 24, cudaMemcpyDeviceToHost, st));
     if (h_iters_done)
         CUDA_TRY(cudaMemcpyAsync(h_iters_done, ctl->iters_done, (size_t)levels * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return DEMONS_OK;
+}
+
+namespace {
+// Second staging slot of demons_register_host_queue, behind the single-registration partition.
+struct QueueSlots {
+    size_t hI[2], hU[2], hUb[2], total;
+};
+QueueSlots queue_slots(const demons_ctx* c, int levels) {
+    const Partition p = make_partition(c, levels, 1);
+    const size_t N = nvox(c->dims);
+    QueueSlots q{};
+    q.hI[0] = p.hI;
+    q.hU[0] = p.hU;
+    q.hUb[0] = p.hUb;
+    size_t off = align_up(p.total);
+    q.hI[1] = off;
+    off += align_up(2 * N * 4);
+    q.hU[1] = off;
+    off += align_up(3 * N * 4);
+    q.hUb[1] = is_ic(c) ? off : 0;
+    if (is_ic(c)) off += align_up(3 * N * 4);
+    q.total = off;
+    return q;
+}
+}  // namespace
+
+size_t demons_workspace_bytes_queue(const demons_ctx* c, int levels) {
+    if (!c || levels < 1 || levels > DEMONS_MAX_LEVELS) return 0;
+    return queue_slots(c, levels).total;
+}
+
+int demons_register_host_queue(demons_ctx* c, int n, const float* const* h_static, const float* const* h_moving,
+                               float* const* h_u, float* const* h_u_back, int levels, const int* h_iters, double eps,
+                               double* h_stats, int* h_iters_done, void* stream) {
+    if (!c) return fail(DEMONS_E_ARG, "ctx is NULL");
+    if (n < 1 || !h_static || !h_moving || !h_u) return fail(DEMONS_E_ARG, "n must be >= 1 and the pointer arrays non-NULL");
+    const bool ic = is_ic(c);
+    if (ic && !h_u_back) return fail(DEMONS_E_ARG, "variant 5 needs h_u_back");
+    if (!ic && h_u_back) return fail(DEMONS_E_ARG, "h_u_back must be NULL unless variant 5");
+    for (int k = 0; k < n; ++k) {
+        const int rc = check_register_args(c, h_static[k], h_moving[k], h_u[k], ic ? h_u_back[k] : nullptr, 1, levels, h_iters);
+        if (rc != DEMONS_OK) return rc;
+    }
+    const QueueSlots q = queue_slots(c, levels);
+    if (q.total > c->ws_bytes)
+        return fail(DEMONS_E_WORKSPACE, "workspace too small: have %zu bytes, need %zu (demons_workspace_bytes_queue)",
+                    c->ws_bytes, q.total);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (!c->q_in) {
+        CUDA_TRY(cudaStreamCreateWithFlags(&c->q_in, cudaStreamNonBlocking));
+        CUDA_TRY(cudaStreamCreateWithFlags(&c->q_out, cudaStreamNonBlocking));
+        for (int k = 0; k < 2; ++k) {
+            CUDA_TRY(cudaEventCreateWithFlags(&c->q_up[k], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&c->q_done[k], cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&c->q_down[k], cudaEventDisableTiming));
+        }
+    }
+    const Partition p = make_partition(c, levels, 1);
+    const size_t N = nvox(c->dims);
+    long long total_iters = 0;
+    for (int l = 0; l < levels; ++l) total_iters += h_iters[l];
+    Control* ctl = reinterpret_cast<Control*>(c->ws + p.control);
+    const bool upload_u = levels == 1 && !c->opt_zero_start;
+    // everything enqueued before this call on `stream` comes first
+    CUDA_TRY(cudaEventRecord(c->q_done[0], st));
+    CUDA_TRY(cudaStreamWaitEvent(c->q_in, c->q_done[0], 0));
+    CUDA_TRY(cudaStreamWaitEvent(c->q_out, c->q_done[0], 0));
+    auto upload = [&](int k) -> int {  // images (and initial fields) of registration k into slot k & 1, on q_in
+        const int s = k & 1;
+        if (k >= 2) {
+            CUDA_TRY(cudaStreamWaitEvent(c->q_in, c->q_done[s], 0));                // registration k - 2 is done with the images
+            if (upload_u) CUDA_TRY(cudaStreamWaitEvent(c->q_in, c->q_down[s], 0));  // and its field has been read back
+        }
+        float* dS = reinterpret_cast<float*>(c->ws + q.hI[s]);
+        CUDA_TRY(cudaMemcpyAsync(dS, h_static[k], N * 4, cudaMemcpyHostToDevice, c->q_in));
+        CUDA_TRY(cudaMemcpyAsync(dS + N, h_moving[k], N * 4, cudaMemcpyHostToDevice, c->q_in));
+        if (upload_u) {
+            CUDA_TRY(cudaMemcpyAsync(c->ws + q.hU[s], h_u[k], 3 * N * 4, cudaMemcpyHostToDevice, c->q_in));
+            if (ic) CUDA_TRY(cudaMemcpyAsync(c->ws + q.hUb[s], h_u_back[k], 3 * N * 4, cudaMemcpyHostToDevice, c->q_in));
+        }
+        CUDA_TRY(cudaEventRecord(c->q_up[s], c->q_in));
+        return DEMONS_OK;
+    };
+    int rc = upload(0);
+    if (rc != DEMONS_OK) return rc;
+    for (int k = 0; k < n; ++k) {
+        const int s = k & 1;
+        if (k + 1 < n && (rc = upload(k + 1)) != DEMONS_OK) return rc;  // rides beside registration k
+        float* dS = reinterpret_cast<float*>(c->ws + q.hI[s]);
+        float* dU = reinterpret_cast<float*>(c->ws + q.hU[s]);
+        float* dUb = ic ? reinterpret_cast<float*>(c->ws + q.hUb[s]) : nullptr;
+        CUDA_TRY(cudaStreamWaitEvent(st, c->q_up[s], 0));
+        if (k >= 2) CUDA_TRY(cudaStreamWaitEvent(st, c->q_down[s], 0));  // the field of registration k - 2 has left the slot
+        rc = register_impl(c, dS, dS + N, dU, dUb, 1, levels, h_iters, eps, nullptr, nullptr, st);
+        if (rc != DEMONS_OK) return rc;
+        if (h_stats && total_iters > 0)
+            CUDA_TRY(cudaMemcpyAsync(h_stats + (size_t)k * total_iters * 3, c->ws + p.stats, (size_t)total_iters * 24,
+                                     cudaMemcpyDeviceToHost, st));
+        if (h_iters_done)
+            CUDA_TRY(cudaMemcpyAsync(h_iters_done + (size_t)k * levels, ctl->iters_done, (size_t)levels * 4,
+                                     cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaEventRecord(c->q_done[s], st));
+        CUDA_TRY(cudaStreamWaitEvent(c->q_out, c->q_done[s], 0));
+        CUDA_TRY(cudaMemcpyAsync(h_u[k], dU, 3 * N * 4, cudaMemcpyDeviceToHost, c->q_out));
+        if (ic) CUDA_TRY(cudaMemcpyAsync(h_u_back[k], dUb, 3 * N * 4, cudaMemcpyDeviceToHost, c->q_out));
+        CUDA_TRY(cudaEventRecord(c->q_down[s], c->q_out));
+    }
+    CUDA_TRY(cudaStreamWaitEvent(st, c->q_down[0], 0));  // `stream` ends behind the last downloads
+    if (n > 1) CUDA_TRY(cudaStreamWaitEvent(st, c->q_down[1], 0));
+    CUDA_TRY(cudaStreamSynchronize(c->q_out));
     CUDA_TRY(cudaStreamSynchronize(st));
     return DEMONS_OK;
 }

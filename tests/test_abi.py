@@ -144,3 +144,32 @@ def test_batch_and_slab_arguments_validated(B):
         assert e.value.code == B.E_ARG
     finally:
         B.demons_destroy(ctx)
+
+
+def test_host_queue_arguments_validated(B):
+    """Host-side validation of demons_register_host_queue (no device needed): the queue workspace is the single
+    registration's plus one more staging slot (2 N floats of images, 3 N of field)."""
+    import numpy as np
+    dims = (16, 12, 10)
+    n_vox = 16 * 12 * 10
+    ctx = B.demons_create(dims, (1.0, 1.0, 1.0), B.PASSIVE, 1.0, 1.0)
+    try:
+        w1, wq = B.demons_workspace_bytes(ctx, 2), B.demons_workspace_bytes_queue(ctx, 2)
+        assert 5 * 4 * n_vox <= wq - w1 <= 5 * 4 * n_vox + 3 * 256
+        assert B.demons_workspace_bytes_queue(ctx, 0) == 0
+        vol = np.zeros((10, 12, 16), np.float32)
+        fld = np.zeros((3, 10, 12, 16), np.float32)
+        with pytest.raises(B.DemonsError) as e:
+            B.demons_register_host_queue(ctx, [], [], [], None, [2, 2])               # empty queue
+        assert e.value.code == B.E_ARG
+        with pytest.raises(B.DemonsError) as e:
+            B.demons_register_host_queue(ctx, [vol], [vol], [fld], [fld], [2, 2])     # u_back for a non-IC variant
+        assert e.value.code == B.E_ARG
+        with pytest.raises(B.DemonsError) as e:
+            B.demons_register_host_queue(ctx, [vol, vol], [vol, vol], [fld, fld], None, [2, -1])
+        assert e.value.code == B.E_ARG
+        with pytest.raises(B.DemonsError) as e:
+            B.demons_register_host_queue(ctx, [vol, vol], [vol, vol], [fld, fld], None, [2, 2])   # no workspace
+        assert e.value.code == B.E_WORKSPACE
+    finally:
+        B.demons_destroy(ctx)

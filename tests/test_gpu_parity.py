@@ -419,6 +419,44 @@ def test_register_batch_sigma2_shares_and_early_stop(torch_cuda, B, P, variant):
     assert min(stops) >= 10, stops
 
 
+@pytest.mark.parametrize("variant,levels", [(0, 1), (3, 2), (5, 2)])
+def test_register_host_queue_equals_single_host_calls(torch_cuda, B, P, variant, levels):
+    """demons_register_host_queue: n registrations from pinned host buffers with the transfers of neighbouring
+    registrations overlapped; every field, statistics row and iteration count equals the demons_register_host call on
+    that pair, bit for bit (two staging slots: five pairs go round the slots more than twice)."""
+    torch = torch_cuda
+    dims = (48, 40, 20)
+    iters = [7] if levels == 1 else [6, 5]
+    alpha = ALPHA.get(variant, 1.0)
+    ic = variant == 5
+    pairs = [P.config1_pair(dims=dims, seed=500 + k, max_norm=1.0 + 0.3 * k)[:2] for k in range(5)]
+    rng = np.random.default_rng(3)
+    u0 = [(0.2 * rng.standard_normal((3,) + pairs[0][0].shape)).astype(np.float32) for _ in pairs]  # used when levels == 1
+    hS = [torch.from_numpy(p[0]).pin_memory() for p in pairs]
+    hM = [torch.from_numpy(p[1]).pin_memory() for p in pairs]
+    hU = [torch.from_numpy(u.copy()).pin_memory() for u in u0]
+    hUb = [torch.from_numpy(-u).pin_memory() for u in u0] if ic else None
+    n = len(pairs)
+    stats = np.zeros((n, int(sum(iters)), 3))
+    done = np.zeros((n, levels), dtype=np.int32)
+    eng = B.Demons(dims, variant=variant, alpha=alpha, levels=levels, queue=True)
+    st = torch.cuda.Stream()
+    B.demons_register_host_queue(eng.ctx, hS, hM, hU, hUb, iters, 0.0, stats, done, st)
+    # the same context still serves the single calls (slot 0 is their staging buffer)
+    for k, (S, M) in enumerate(pairs):
+        hu = u0[k].copy()
+        hub = -u0[k] if ic else None
+        s1 = np.zeros((int(sum(iters)), 3))
+        d1 = np.zeros(levels, dtype=np.int32)
+        B.demons_register_host(eng.ctx, S, M, hu, hub, iters, 0.0, s1, d1, st)
+        assert np.array_equal(hU[k].numpy(), hu), f"pair {k}"
+        if ic:
+            assert np.array_equal(hUb[k].numpy(), hub), f"pair {k} (backward field)"
+        assert np.array_equal(stats[k], s1) and done[k].tolist() == d1.tolist()
+        assert np.abs(hu).max() > 0
+    eng.close()
+
+
 def test_inverse_consistent_one_field_is_bit_identical(torch_cuda, B, P, oracle):
     """Variant 5 from a zero start iterates on u_f alone (u_b = -u_f, pin P10) and writes u_b on exit: same
     bits, fields and statistics, as iterating on both fields ("ic_one_field" = 0)."""
