@@ -885,34 +885,41 @@ int demons_register_host_queue(demons_ctx* c, int n, const float* const* h_stati
         CUDA_TRY(cudaEventRecord(c->q_up[s], c->q_in));
         return DEMONS_OK;
     };
-    int rc = upload(0);
-    if (rc != DEMONS_OK) return rc;
-    for (int k = 0; k < n; ++k) {
-        const int s = k & 1;
-        if (k + 1 < n && (rc = upload(k + 1)) != DEMONS_OK) return rc;  // rides beside registration k
-        float* dS = reinterpret_cast<float*>(c->ws + q.hI[s]);
-        float* dU = reinterpret_cast<float*>(c->ws + q.hU[s]);
-        float* dUb = ic ? reinterpret_cast<float*>(c->ws + q.hUb[s]) : nullptr;
-        CUDA_TRY(cudaStreamWaitEvent(st, c->q_up[s], 0));
-        if (k >= 2) CUDA_TRY(cudaStreamWaitEvent(st, c->q_down[s], 0));  // the field of registration k - 2 has left the slot
-        rc = register_impl(c, dS, dS + N, dU, dUb, 1, levels, h_iters, eps, nullptr, nullptr, st);
+    auto enqueue_all = [&]() -> int {
+        int rc = upload(0);
         if (rc != DEMONS_OK) return rc;
-        if (h_stats && total_iters > 0)
-            CUDA_TRY(cudaMemcpyAsync(h_stats + (size_t)k * total_iters * 3, c->ws + p.stats, (size_t)total_iters * 24,
-                                     cudaMemcpyDeviceToHost, st));
-        if (h_iters_done)
-            CUDA_TRY(cudaMemcpyAsync(h_iters_done + (size_t)k * levels, ctl->iters_done, (size_t)levels * 4,
-                                     cudaMemcpyDeviceToHost, st));
-        CUDA_TRY(cudaEventRecord(c->q_done[s], st));
-        CUDA_TRY(cudaStreamWaitEvent(c->q_out, c->q_done[s], 0));
-        CUDA_TRY(cudaMemcpyAsync(h_u[k], dU, 3 * N * 4, cudaMemcpyDeviceToHost, c->q_out));
-        if (ic) CUDA_TRY(cudaMemcpyAsync(h_u_back[k], dUb, 3 * N * 4, cudaMemcpyDeviceToHost, c->q_out));
-        CUDA_TRY(cudaEventRecord(c->q_down[s], c->q_out));
-    }
-    CUDA_TRY(cudaStreamWaitEvent(st, c->q_down[0], 0));  // `stream` ends behind the last downloads
-    if (n > 1) CUDA_TRY(cudaStreamWaitEvent(st, c->q_down[1], 0));
-    CUDA_TRY(cudaStreamSynchronize(c->q_out));
-    CUDA_TRY(cudaStreamSynchronize(st));
+        for (int k = 0; k < n; ++k) {
+            const int s = k & 1;
+            if (k + 1 < n && (rc = upload(k + 1)) != DEMONS_OK) return rc;  // rides beside registration k
+            float* dS = reinterpret_cast<float*>(c->ws + q.hI[s]);
+            float* dU = reinterpret_cast<float*>(c->ws + q.hU[s]);
+            float* dUb = ic ? reinterpret_cast<float*>(c->ws + q.hUb[s]) : nullptr;
+            CUDA_TRY(cudaStreamWaitEvent(st, c->q_up[s], 0));
+            if (k >= 2) CUDA_TRY(cudaStreamWaitEvent(st, c->q_down[s], 0));  // the field of registration k - 2 has left the slot
+            rc = register_impl(c, dS, dS + N, dU, dUb, 1, levels, h_iters, eps, nullptr, nullptr, st);
+            if (rc != DEMONS_OK) return rc;
+            if (h_stats && total_iters > 0)
+                CUDA_TRY(cudaMemcpyAsync(h_stats + (size_t)k * total_iters * 3, c->ws + p.stats, (size_t)total_iters * 24,
+                                         cudaMemcpyDeviceToHost, st));
+            if (h_iters_done)
+                CUDA_TRY(cudaMemcpyAsync(h_iters_done + (size_t)k * levels, ctl->iters_done, (size_t)levels * 4,
+                                         cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(cudaEventRecord(c->q_done[s], st));
+            CUDA_TRY(cudaStreamWaitEvent(c->q_out, c->q_done[s], 0));
+            CUDA_TRY(cudaMemcpyAsync(h_u[k], dU, 3 * N * 4, cudaMemcpyDeviceToHost, c->q_out));
+            if (ic) CUDA_TRY(cudaMemcpyAsync(h_u_back[k], dUb, 3 * N * 4, cudaMemcpyDeviceToHost, c->q_out));
+            CUDA_TRY(cudaEventRecord(c->q_down[s], c->q_out));
+        }
+        CUDA_TRY(cudaStreamWaitEvent(st, c->q_down[0], 0));  // `stream` ends behind the last downloads
+        if (n > 1) CUDA_TRY(cudaStreamWaitEvent(st, c->q_down[1], 0));
+        return DEMONS_OK;
+    };
+    const int rq = enqueue_all();
+    // drain the three streams whatever happened: the caller's buffers must not be in flight when this call returns
+    const cudaError_t e_in = cudaStreamSynchronize(c->q_in), e_out = cudaStreamSynchronize(c->q_out), e_st = cudaStreamSynchronize(st);
+    if (rq != DEMONS_OK) return rq;
+    if (e_in != cudaSuccess || e_out != cudaSuccess || e_st != cudaSuccess)
+        return fail(DEMONS_E_CUDA, "queue synchronise failed: %s", cudaGetErrorString(e_in != cudaSuccess ? e_in : e_out != cudaSuccess ? e_out : e_st));
     return DEMONS_OK;
 }
 
