@@ -244,6 +244,31 @@ int demons_cc(demons_ctx* ctx, const int dims[3], const float* d_static, const f
 int demons_point_error(demons_ctx* ctx, const int dims[3], const float* d_u, int n_points,
                        const float* d_points, const float* d_expect, double* d_err, void* stream);
 
+/* ---- the one entry point that needs no workspace and allocates nothing ------------------------------------
+ * demons_ssd_static computes what demons_ssd computes -- sum (warp(M,u) - S)^2, or with d_ub != NULL the two-field
+ * form sum (warp(M,u) - warp(S,ub))^2 of variant 5 (reading O8) -- for callers who cannot
+ * give the library device memory of their own: a plug-in inside an application that owns the device's memory
+ * budget and forbids cudaMalloc, a checking hook that must leave the process's footprint as it found it, a
+ * time-critical loop in which an allocator call would stall every stream of the device.  It takes no context:
+ * inputs and the one output double are the caller's, everything else it needs is a scratch array compiled into the
+ * library (128 KiB + 256 B of global memory on every GPU that loads libdemons.so, held until the process ends).
+ * The call makes no cudaMalloc / cudaFree and uses no allocating library routine; it enqueues one 4-byte
+ * memset and one kernel on `stream` and returns without synchronising.
+ *  - Limit: nx*ny*nz <= DEMONS_SSD_STATIC_MAX_VOXELS (one scratch slot per 4096 voxels).  Anything larger is
+ *    refused with DEMONS_E_UNSUPPORTED and a message that names both numbers; use demons_ssd then.
+ *  - First call on a device: looks up the scratch array's device address (once per device, with that device
+ *    current, kept for the life of the process).  Make that first call outside any stream capture.
+ *  - All calls on a device share the one array.  Two calls whose kernels may run at the same time (different
+ *    streams, or host threads that do not order their work) overwrite each other's partial sums and give wrong
+ *    results: order them on one stream or with events.  Back-to-back calls on one stream are fine; each call
+ *    re-zeroes the only word that must start at zero.
+ *  - Result: agrees with demons_ssd to rounding of a double sum (the block partition differs: here it depends on
+ *    the volume only, so the same inputs give the same bits on any GPU).
+ * d_static, d_moving: [N] floats; d_u (d_ub): [3][N] floats; d_out: 1 double; all DEVICE pointers. */
+#define DEMONS_SSD_STATIC_MAX_VOXELS 67108864 /* 2^26 = 512 x 512 x 256 */
+int demons_ssd_static(const int dims[3], const float* d_static, const float* d_moving, const float* d_u,
+                      const float* d_ub, double* d_out, void* stream);
+
 /* Thread-local description of the last failure on this thread ("" if none). */
 const char* demons_last_error(void);
 

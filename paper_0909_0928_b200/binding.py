@@ -52,6 +52,7 @@ SIGNATURES = {
     "demons_ic_error": (ctypes.c_int, [_vp, _c_int3, _vp, _vp, _vp, _vp]),
     "demons_cc": (ctypes.c_int, [_vp, _c_int3, _vp, _vp, _vp, _vp, _vp, _vp]),
     "demons_point_error": (ctypes.c_int, [_vp, _c_int3, _vp, ctypes.c_int, _vp, _vp, _vp, _vp]),
+    "demons_ssd_static": (ctypes.c_int, [_c_int3, _vp, _vp, _vp, _vp, _vp, _vp]),
     "demons_last_error": (ctypes.c_char_p, []),
 }
 
@@ -244,6 +245,15 @@ def demons_cc(ctx, dims, d_static, d_moving, d_u, d_ub, d_out, stream=None):
 def demons_point_error(ctx, dims, d_u, n_points, d_points, d_expect, d_err, stream=None):
     _check(lib().demons_point_error(ctx, _int3(dims), _ptr(d_u), int(n_points), _ptr(d_points), _ptr(d_expect),
                                     _ptr(d_err), _stream(stream)))
+
+
+SSD_STATIC_MAX_VOXELS = 1 << 26
+
+
+def demons_ssd_static(dims, d_static, d_moving, d_u, d_ub, d_out, stream=None):
+    """SSD without a context or a workspace (scratch is a fixed array inside libdemons.so); see include/demons.h."""
+    _check(lib().demons_ssd_static(_int3(dims), _ptr(d_static), _ptr(d_moving), _ptr(d_u), _ptr(d_ub), _ptr(d_out),
+                                   _stream(stream)))
 
 
 def demons_last_error():

@@ -16,7 +16,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdemons.so")
 OBJ_DIR = os.path.join(HERE, "build")
-SOURCES = ["demons_api.cu", "warp_force.cu", "smooth.cu", "smooth_tma.cu", "pyramid.cu", "reduce.cu"]
+SOURCES = ["demons_api.cu", "warp_force.cu", "smooth.cu", "smooth_tma.cu", "pyramid.cu", "reduce.cu", "ssd_static.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--use_fast_math=false"]
 

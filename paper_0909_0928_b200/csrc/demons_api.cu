@@ -63,6 +63,10 @@ struct GraphEntry {
 
 }  // namespace
 
+namespace demons {
+void set_last_error(const char* msg) { g_last_error = msg ? msg : ""; }
+}  // namespace demons
+
 struct demons_ctx {
     Dims dims;
     float spacing[3];

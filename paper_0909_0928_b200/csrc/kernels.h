@@ -93,6 +93,9 @@ int launch_cc(const Dims& d, const float* S, const float* M, const float* u, con
 int launch_point_error(const Dims& d, const float spacing[3], const float* u, int n, const float* points,
                        const float* expect, double* err, cudaStream_t stream);
 
+// Stores `msg` as this thread's demons_last_error() text (for entry points that live outside demons_api.cu).
+void set_last_error(const char* msg);
+
 // Per-device properties, cached per device ordinal (a process may drive several devices).
 int sm_count();
 size_t max_policy_window();
