@@ -13,13 +13,14 @@ field, the final SSD and, for config 4, the inverse-consistency error); "batch" 
 demons_register_batch on config 3 (B = 1, 4, 16 pairs per call); "evaluation" holds the accuracy
 protocol for the timed config-2 registration.
 
-"roofline" is per kernel.  The duration of a kernel inside the graph-replayed iteration is not observable
-from the host, so it is ATTRIBUTED: (the kernel's share of the iteration) x (the iteration time of the
-timed region, CUDA events on the launching stream).  Two shares are reported: from the event-bracketed
-profile pass of this run ("share_events") and from the committed ncu launch list of this same command
-("share_ncu", profiles/r02_kernel_shares.csv); `frac` uses the ncu share when the file is there.
+"roofline" is per kernel, and the kernel durations are MEASURED IN THIS RUN from inside the replayed graph: with the
+library's "profile" = 2 option one iteration in the middle of every 20-iteration graph chunk carries CUDA event-record
+nodes (before the force kernel, between force and smoother, after the smoother); `avg_ms` is their mean over three
+registrations (45 replays).  `frac` depends on nothing under profiles/.  Beside it, as cross-checks only: the share of
+the iteration from the event-bracketed no-graph pass ("share_events_no_graph"), the committed ncu share
+("share_ncu_committed") and "stale_share" = true when the committed share is more than 0.05 away from this run's.
 "achieved" = ALGORITHMIC bytes / that duration (an effective bandwidth: each array element once);
-"hbm_measured" = the DRAM bytes ncu counted for that kernel (profiles/r02_ncu_traffic.csv) / the same
+"hbm_measured" = the DRAM bytes ncu counted for that kernel (profiles/r0N_ncu_traffic.csv) / the same
 duration -- real HBM traffic, lower, because part of the field is still in L2 between the two kernels.
 Both are given as fractions of the measured copy peak (MEASURED_PEAKS.json) and of the nominal 8 TB/s.
 
@@ -213,7 +214,8 @@ def relaunch_under_torchrun(args):
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
     env = dict(os.environ)
-    env.setdefault("NCCL_DEBUG", "WARN")
+    env.setdefault("NCCL_DEBUG", "INFO")          # the communicator lines (comm ... nranks N) print at INFO only
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
     return subprocess.call(cmd, env=env)
 
 
@@ -443,40 +445,71 @@ def main():
     torch.cuda.synchronize()
     prof = B.demons_get_profile(eng.ctx)
     launches_per_iter = (B.demons_launch_count(eng.ctx) - l0) / sum(ITERS)
+    # ---- the same kernels timed INSIDE the replayed graph ("profile" = 2: event-record nodes around one iteration in
+    # the middle of every 20-iteration chunk): this, and nothing read from profiles/, is what `frac` is computed from
+    B.demons_set_option(eng.ctx, "profile", 2)
+    ingraph = {"force": {"ms": 0.0, "groups": 0}, "smooth": {"ms": 0.0, "groups": 0}, "warp": {"ms": 0.0, "groups": 0}}
+    for _ in range(3):
+        du.zero_()
+        torch.cuda.synchronize()
+        B.demons_register(eng.ctx, dS, dM, du, None, ITERS, 0.0, None, None, stream)
+        torch.cuda.synchronize()
+        got = B.demons_get_profile(eng.ctx)
+        for k in ingraph:
+            ingraph[k]["ms"] += got[k]["ms"]
+            ingraph[k]["groups"] += got[k]["groups"]
     B.demons_set_option(eng.ctx, "profile", 0)
+    assert ingraph["force"]["groups"] > 0 and ingraph["smooth"]["groups"] > 0, "in-graph timing returned nothing"
     smooth_launches = launches_per_iter - 2  # per iteration: the force kernel, k_metrics_final (side branch), the smoother
     bytes_per_voxel = {"force": 32.0, "smooth": 24.0 if smooth_launches <= 1 else 72.0}
     kernel_names = {"force": "k_force_fixed_lc<0,4> (fused warp+gradient+force+update+metrics, lane-consecutive cells)",
                     "smooth": "k_smooth_tma<3> (TMA-fed single pass, 3 components)" if smooth_launches <= 1
                     else "k_smooth_axis x3 (separable fallback, 3 components)"}
     peak, peak_src = measured_peak()
-    ncu_share = committed_csv("r02_kernel_shares.csv")    # this command under ncu --metrics gpu__time_duration.sum
-    ncu_bytes = committed_csv("r02_ncu_traffic.csv")      # this command under ncu --set full
+    # cross-checks only (side fields): ncu's share of the iteration and DRAM bytes per launch from committed captures
+    ncu_share = committed_csv("r03_kernel_shares.csv") or committed_csv("r02_kernel_shares.csv")
+    ncu_bytes = committed_csv("r03_ncu_traffic.csv") or committed_csv("r02_ncu_traffic.csv")
     per_kernel = {}
     ms_per_iter = 1e3 * agg["seconds"] / (args.steps * sum(ITERS))
+    node_gap_ms = ingraph["warp"]["ms"] / max(ingraph["warp"]["groups"], 1)   # the empty bracket of "profile" = 2
+    ingraph_iter = sum(ingraph[k]["ms"] / ingraph[k]["groups"] for k in ("force", "smooth"))
     for k in ("force", "smooth"):
         ms_raw = prof[k]["ms"] / max(prof[k]["groups"], 1)
         share_ev = prof[k]["ms"] / max(prof["force"]["ms"] + prof["smooth"]["ms"], 1e-9)
-        share = ncu_share.get(k, share_ev)
-        ms = share * ms_per_iter
+        ms = ingraph[k]["ms"] / ingraph[k]["groups"]
+        share_ingraph = ms / ingraph_iter
         gbs = bytes_per_voxel[k] * N / (ms * 1e-3) / 1e9 if ms > 0 else 0.0
-        entry = {"kernel": kernel_names[k], "avg_ms": ms, "avg_ms_how": "share x iteration time of the timed region (graph replay)",
-                 "share_used": share, "share_events": share_ev, "share_ncu": ncu_share.get(k),
-                 "avg_ms_event_bracketed": ms_raw, "alg_bytes_per_voxel": bytes_per_voxel[k],
+        entry = {"kernel": kernel_names[k], "avg_ms": ms,
+                 "avg_ms_how": "measured in this run: CUDA event-record nodes inside the replayed level graph around one "
+                               f"iteration per 20-iteration chunk, mean of {ingraph[k]['groups']} replays (includes the "
+                               "node-to-node launch gaps on both sides of the kernel)",
+                 "share_ingraph": share_ingraph, "avg_ms_share_x_iteration": share_ingraph * ms_per_iter,
+                 "event_node_gap_ms": node_gap_ms,
+                 "share_events_no_graph": share_ev, "share_ncu_committed": ncu_share.get(k),
+                 "avg_ms_event_bracketed_no_graph": ms_raw, "alg_bytes_per_voxel": bytes_per_voxel[k],
                  "achieved_gbs": gbs, "achieved_kind": "effective (algorithmic bytes / time)",
                  "frac": gbs / peak, "frac_of_nominal": gbs / NOMINAL_HBM_GBS}
         if k in ncu_bytes and ms > 0:
             dram = ncu_bytes[k] / (ms * 1e-3) / 1e9
             entry["hbm_measured"] = {"dram_bytes_per_launch": ncu_bytes[k], "gbs": dram, "frac": dram / peak,
                                      "frac_of_nominal": dram / NOMINAL_HBM_GBS,
-                                     "note": "ncu dram__bytes_read + dram__bytes_write of this kernel / the same duration"}
+                                     "note": "committed ncu dram__bytes_read + dram__bytes_write of this kernel / the "
+                                             "duration measured in this run"}
         per_kernel[k] = entry
+    # the committed ncu shares are only a cross-check; say so loudly when they no longer describe this build
+    stale_share = bool(ncu_share) and any(abs(ncu_share.get(k, per_kernel[k]["share_ingraph"]) - per_kernel[k]["share_ingraph"]) > 0.05
+                                          for k in per_kernel)
     dom = max(("force", "smooth"), key=lambda k: per_kernel[k]["avg_ms"])
     it_gbs = (bytes_per_voxel["force"] + bytes_per_voxel["smooth"]) * N / (ms_per_iter * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": per_kernel[dom]["kernel"], "achieved": per_kernel[dom]["achieved_gbs"],
                 "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": per_kernel[dom]["frac"],
                 "frac_of_nominal": per_kernel[dom]["frac_of_nominal"], "nominal_peak": NOMINAL_HBM_GBS,
                 "traffic": ncu_bytes.get(dom),
+                "stale_share": stale_share,
+                "ingraph_iteration_ms": ingraph_iter, "event_node_gap_ms": node_gap_ms,
+                "note": "frac uses the raw in-graph interval, record-node gaps included (event_node_gap_ms = an empty "
+                        "bracket measured the same way): the timed iteration is longer than the untimed one "
+                        "(whole_iteration.ms), so frac is a lower bound",
                 "whole_iteration": {"ms": ms_per_iter, "alg_bytes_per_voxel": bytes_per_voxel["force"] + bytes_per_voxel["smooth"],
                                     "achieved_gbs": it_gbs, "frac": it_gbs / peak, "frac_of_nominal": it_gbs / NOMINAL_HBM_GBS,
                                     "note": "driver-timed: no attribution involved"},

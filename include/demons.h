@@ -95,16 +95,23 @@ long long demons_launch_count(const demons_ctx* ctx);
 /* "profile" option: after a demons_register call made with the option on, the summed device time
  * (ms, CUDA events on the caller's stream) and the number of timed groups per kernel class:
  * [0] force kernels (fused warp+force+update, or the force pass of variants 2-5), [1] the warp
- * pass of variants 2-5, [2] smoothing, [3] pyramid (restrict + prolong). */
+ * pass of variants 2-5, [2] smoothing, [3] pyramid (restrict + prolong).
+ * With "profile" = 2 the registration keeps replaying its level graphs, and ONE iteration in the middle of every
+ * replayed chunk of 20 carries three event-record nodes (before the force kernel(s), between force and smoothing,
+ * after the smoothing kernel(s)): [0] is then the time from the first to the second (variants 2-5: warp pass and
+ * force pass together), [2] from the second to the third, each summed over the replays (groups = replays); [1] is
+ * an EMPTY bracket in this mode -- a fourth record node directly behind the third -- i.e. what one record node adds
+ * to each of the two intervals; the host reads the events after every replay (one stream synchronise per 20 iterations), [3] is not
+ * timed.  These are the durations of the kernels as the run executes them -- warm L2, neighbours in flight. */
 int demons_get_profile(const demons_ctx* ctx, double h_ms[4], long long h_launch_groups[4]);
 
 /* Named integer options.  "graphs" (default 1): replay the per-level iteration through a CUDA
  * graph.  "texture" (default 0): S9, sample the moving image through the texture unit with
  * hardware linear filtering (PAPER.md L181 reports its precision as insufficient; measured
  * option only -- fails parity by design).  "generic_smooth" (default 0): always use
- * the three separable smoothing passes instead of the fused kernel.  "profile" (default 0): time
+ * the three separable smoothing passes instead of the fused kernel.  "profile" (default 0): 1 = time
  * every kernel class with events inside demons_register (disables graphs, adds a final
- * synchronise; see demons_get_profile).  "zero_start" (default 0): a single-level registration starts
+ * synchronise; see demons_get_profile); 2 = time one iteration per replayed graph chunk from inside the graph.  "zero_start" (default 0): a single-level registration starts
  * from a zero field set on the device; d_u / h_u (and u_back) are then outputs only and
  * demons_register_host does not upload them.  "l2_persist" (default 1): the kernels that gather from the
  * moving image launch with an access-policy window that asks L2 to keep that image resident

@@ -56,6 +56,8 @@ struct GraphEntry {
     const float *S, *M;
     float *u, *ub;
     int chunk, nb, one_field;
+    int timed;         // "profile" = 2: one iteration of the chunk carries event-record nodes
+    int b0, nb_total;  // the captured kernels carry workspace offsets that move with the pair index and the batch size
     double eps;
     cudaGraphExec_t exec;
     int launches;
@@ -88,6 +90,7 @@ struct demons_ctx {
     size_t l2_prev_limit = 0;
     std::vector<cudaEvent_t> prof_all;                               // events of the profiled call
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_pairs[4];  // per kernel class: start/stop
+    cudaEvent_t tg[4] = {nullptr, nullptr, nullptr, nullptr};  // "profile" = 2: before force / between / after the smoother / once more, recorded by graph nodes
     double prof_ms[4] = {0, 0, 0, 0};
     long long prof_n[4] = {0, 0, 0, 0};
     std::vector<GraphEntry> graphs;
@@ -308,7 +311,7 @@ enum { PROF_FORCE = 0, PROF_WARP = 1, PROF_SMOOTH = 2, PROF_PYRAMID = 3 };
 
 // "profile" option: bracket every launch of a kernel class with a pair of events on the stream.
 cudaEvent_t prof_event(demons_ctx* c, cudaStream_t st, bool record) {
-    if (!c->opt_profile) return nullptr;
+    if (c->opt_profile != 1) return nullptr;
     cudaEvent_t e = nullptr;
     if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
     if (record) cudaEventRecord(e, st);
@@ -347,6 +350,7 @@ struct LevelBuffers {
     float* u;           // [nb][3][n]
     float* ub;          // variant 5, two-field form; nullptr otherwise
     int b0, nb;         // first pair and number of pairs of the group
+    int nb_total;       // pairs of the whole call (the workspace partition is laid out for this many)
     int one_field;
 };
 
@@ -361,7 +365,7 @@ int ensure_side(demons_ctx* c) {
 
 // One iteration of a group of pairs: [warp_force ; smooth the total field] (reading C2).
 int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb, const L2Window& win, double eps,
-                      cudaStream_t st, int* launches) {
+                      cudaStream_t st, int* launches, bool timed = false) {
     const bool ic = is_ic(c);
     const bool two = ic && !lb.one_field;
     const size_t N = nvox(c->dims);
@@ -388,6 +392,9 @@ int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb,
     fa.l2_ptr = win.ptr;
     fa.l2_bytes = win.bytes;
     fa.l2_ratio = win.ratio;
+    // timed (inside a stream capture only): event-record NODES around the kernels of this iteration, so that the
+    // replayed graph itself says how long they take with the caches and clocks of the run
+    if (timed) CUDA_TRY(cudaEventRecordWithFlags(c->tg[0], st, cudaEventRecordExternal));
     cudaEvent_t e0 = prof_event(c, st, true);
     fa.ev_mid = c->variant >= DEMONS_ACTIVE ? prof_event(c, st, false) : nullptr;
     int metric_blocks = 0;
@@ -395,6 +402,7 @@ int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb,
     int k = launch_warp_force(fa, st);
     if (k < 0) return fail(DEMONS_E_CUDA, "warp_force launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     *launches += k;
+    if (timed) CUDA_TRY(cudaEventRecordWithFlags(c->tg[1], st, cudaEventRecordExternal));
     cudaEvent_t e1 = prof_event(c, st, true);
     if (fa.ev_mid) {
         prof_pair(c, PROF_WARP, e0, fa.ev_mid);
@@ -431,6 +439,10 @@ int enqueue_iteration(demons_ctx* c, const Partition& p, const LevelBuffers& lb,
         if (k < 0) return fail(DEMONS_E_CUDA, "smooth launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         *launches += k;
     }
+    if (timed) {
+        CUDA_TRY(cudaEventRecordWithFlags(c->tg[2], st, cudaEventRecordExternal));  // end of the smoothing kernel(s)
+        CUDA_TRY(cudaEventRecordWithFlags(c->tg[3], st, cudaEventRecordExternal));  // empty bracket: what a record node costs
+    }
     CUDA_TRY(cudaStreamWaitEvent(st, c->ev_join, 0));  // join: the next force kernel reads the stop flag
     prof_pair(c, PROF_SMOOTH, e1, prof_event(c, st, true));
     return DEMONS_OK;
@@ -450,12 +462,13 @@ int run_level(demons_ctx* c, const Partition& p, const LevelBuffers& lb, int ite
         c->launches += 1;
     }
     const int chunk = iters >= 20 ? 20 : iters;
-    if (c->opt_graphs && capturable(st) && iters >= 4 && !c->opt_texture && !c->opt_profile) {
+    if (c->opt_graphs && capturable(st) && iters >= 4 && !c->opt_texture && c->opt_profile != 1) {
+        const int timed = c->opt_profile == 2 ? 1 : 0;
         GraphEntry* ge = nullptr;
         for (auto& g : c->graphs)
             if (g.d.nx == lb.d.nx && g.d.ny == lb.d.ny && g.d.nz == lb.d.nz && g.S == lb.S && g.M == lb.M &&
                 g.u == lb.u && g.ub == lb.ub && g.chunk == chunk && g.eps == eps && g.nb == lb.nb &&
-                g.one_field == lb.one_field)
+                g.one_field == lb.one_field && g.b0 == lb.b0 && g.nb_total == lb.nb_total && g.timed == timed)
                 ge = &g;
         if (!ge) {
             GraphEntry g{};
@@ -468,10 +481,15 @@ int run_level(demons_ctx* c, const Partition& p, const LevelBuffers& lb, int ite
             g.eps = eps;
             g.nb = lb.nb;
             g.one_field = lb.one_field;
+            g.b0 = lb.b0;
+            g.nb_total = lb.nb_total;
+            g.timed = timed;
             cudaGraph_t graph = nullptr;
             CUDA_TRY(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
             int rc = DEMONS_OK;
-            for (int i = 0; i < chunk && rc == DEMONS_OK; ++i) rc = enqueue_iteration(c, p, lb, win, eps, st, &g.launches);
+            // the timed iteration sits in the middle of the chunk, with replayed work on both sides of it
+            for (int i = 0; i < chunk && rc == DEMONS_OK; ++i)
+                rc = enqueue_iteration(c, p, lb, win, eps, st, &g.launches, timed && i == chunk / 2);
             cudaError_t e = cudaStreamEndCapture(st, &graph);
             if (rc != DEMONS_OK) {
                 if (graph) cudaGraphDestroy(graph);
@@ -492,6 +510,19 @@ int run_level(demons_ctx* c, const Partition& p, const LevelBuffers& lb, int ite
             CUDA_TRY(cudaGraphLaunch(ge->exec, st));
             c->launches += ge->launches;
             done += chunk;
+            if (timed) {  // read the three events of this replay before the next one records them again
+                CUDA_TRY(cudaStreamSynchronize(st));
+                float t_force = 0.f, t_smooth = 0.f, t_empty = 0.f;
+                CUDA_TRY(cudaEventElapsedTime(&t_force, c->tg[0], c->tg[1]));
+                CUDA_TRY(cudaEventElapsedTime(&t_smooth, c->tg[1], c->tg[2]));
+                CUDA_TRY(cudaEventElapsedTime(&t_empty, c->tg[2], c->tg[3]));
+                c->prof_ms[PROF_FORCE] += t_force;
+                c->prof_ms[PROF_SMOOTH] += t_smooth;
+                c->prof_ms[PROF_WARP] += t_empty;  // slot [1] carries the empty bracket in this mode
+                c->prof_n[PROF_FORCE] += 1;
+                c->prof_n[PROF_SMOOTH] += 1;
+                c->prof_n[PROF_WARP] += 1;
+            }
         }
     }
     for (; done < iters; ++done) {
@@ -506,9 +537,14 @@ int run_level(demons_ctx* c, const Partition& p, const LevelBuffers& lb, int ite
 // Pairs per launch on a level of n voxels: enough voxels per launch to fill the GPU (a 256x256x100 level
 // does; a 64x64x25 level needs the whole batch), never more than the batch.  Large levels run pair by pair:
 // their launches already fill the machine and the images of ONE pair stay resident in L2.
-int group_size(size_t n, int nb) {
+int group_size(size_t n, int nb, int nz = 1) {
     const size_t target = (size_t)3 << 20;  // voxels per launch
     size_t g = (target + n - 1) / n;
+    // the separable smoothing fallback and the scalar |grad M|^2 kernel carry (planes x components x pairs) in
+    // gridDim.z (<= 65535): a thin, tall level that misses the fast paths must not fail as a batch where every pair
+    // alone succeeds
+    const size_t zcap = (size_t)65535 / ((size_t)3 * (size_t)(nz < 1 ? 1 : nz));
+    if (g > zcap) g = zcap;
     if (g < 1) g = 1;
     if (g > (size_t)nb) g = nb;
     return (int)g;
@@ -528,6 +564,11 @@ int register_impl(demons_ctx* c, const float* dS, const float* dM, float* du, fl
     // iterated on and u_b is written once on exit; bit-identical to iterating on both fields
     const int one_field = ic && zero_start && c->opt_ic_one_field ? 1 : 0;
     prof_clear(c);
+    if (c->opt_profile == 2) {
+        for (int k = 0; k < 4; ++k) c->prof_ms[k] = 0.0, c->prof_n[k] = 0;
+        for (int k = 0; k < 4; ++k)
+            if (!c->tg[k]) CUDA_TRY(cudaEventCreate(&c->tg[k]));
+    }
     if (const int rs = ensure_side(c); rs != DEMONS_OK) return rs;
     CUDA_TRY(cudaMemsetAsync(ctl, 0, (size_t)nb * sizeof(Control), st));
     if (total_iters > 0)
@@ -566,7 +607,7 @@ int register_impl(demons_ctx* c, const float* dS, const float* dM, float* du, fl
     for (int step = 0; step < levels; ++step) {
         const int l = levels - 1 - step;  // coarse -> fine
         const size_t n = nvox(lv[l].d);
-        const int G = group_size(n, nb);
+        const int G = group_size(n, nb, lv[l].d.nz);
         if (step > 0)  // level_iter, stop_force, stop_smooth of every pair
             CUDA_TRY(cudaMemset2DAsync(&ctl[0].level_iter, sizeof(Control), 0, 12, nb, st));
         for (int b0 = 0; b0 < nb; b0 += G) {
@@ -579,6 +620,7 @@ int register_impl(demons_ctx* c, const float* dS, const float* dM, float* du, fl
             lb.u = lv[l].u + (size_t)b0 * 3 * n;
             lb.ub = ic && !one_field ? lv[l].ub + (size_t)b0 * 3 * n : nullptr;
             lb.b0 = b0;
+            lb.nb_total = nb;
             lb.nb = g;
             lb.one_field = one_field;
             if (c->opt_texture) {
@@ -616,7 +658,7 @@ int register_impl(demons_ctx* c, const float* dS, const float* dM, float* du, fl
         CUDA_TRY(cudaMemcpy2DAsync(h_done, (size_t)levels * 4, ctl[0].iters_done, sizeof(Control), (size_t)levels * 4, nb,
                                    cudaMemcpyDeviceToHost, st));
     if (h_stats || h_done || c->opt_profile) CUDA_TRY(cudaStreamSynchronize(st));
-    if (c->opt_profile) prof_collect(c);
+    if (c->opt_profile == 1) prof_collect(c);
     return DEMONS_OK;
 }
 
@@ -636,7 +678,7 @@ int check_register_args(demons_ctx* c, const void* S, const void* M, const void*
     }
     if (total > DEMONS_MAX_STATS_ROWS) return fail(DEMONS_E_ARG, "more than DEMONS_MAX_STATS_ROWS iterations");
     if (nb > 1 && c->opt_texture) return fail(DEMONS_E_UNSUPPORTED, "the texture option serves single registrations only");
-    if (nb > 1 && (double)nb * (double)nvox(c->dims) >= 2147483647.0 / 4.0 && group_size(nvox(c->dims), nb) > 1)
+    if (nb > 1 && (double)nb * (double)nvox(c->dims) >= 2147483647.0 / 4.0 && group_size(nvox(c->dims), nb, c->dims.nz) > 1)
         return fail(DEMONS_E_UNSUPPORTED, "batch too large for 32-bit indexing");
     return check_ws(c, levels, nb);
 }
@@ -681,6 +723,8 @@ void demons_destroy(demons_ctx* c) {
         cudaGetLastError();
     }
     for (auto& g : c->graphs) cudaGraphExecDestroy(g.exec);
+    for (cudaEvent_t e : c->tg)
+        if (e) cudaEventDestroy(e);
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
     if (c->side) cudaStreamDestroy(c->side);
@@ -747,7 +791,7 @@ int demons_set_option(demons_ctx* c, const char* name, int value) {
     if (!strcmp(name, "graphs")) c->opt_graphs = value != 0;
     else if (!strcmp(name, "texture")) c->opt_texture = value != 0;
     else if (!strcmp(name, "generic_smooth")) c->opt_generic_smooth = value != 0;
-    else if (!strcmp(name, "profile")) c->opt_profile = value != 0;
+    else if (!strcmp(name, "profile")) c->opt_profile = value == 2 ? 2 : (value != 0);
     else if (!strcmp(name, "l2_persist")) c->opt_l2_persist = value != 0;
     else if (!strcmp(name, "zero_start")) c->opt_zero_start = value != 0;
     else if (!strcmp(name, "ic_one_field")) c->opt_ic_one_field = value != 0;
@@ -855,12 +899,26 @@ int demons_register_host_queue(demons_ctx* c, int n, const float* const* h_stati
                     c->ws_bytes, q.total);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (!c->q_in) {
-        CUDA_TRY(cudaStreamCreateWithFlags(&c->q_in, cudaStreamNonBlocking));
-        CUDA_TRY(cudaStreamCreateWithFlags(&c->q_out, cudaStreamNonBlocking));
+        // all eight objects or none: created into locals and handed to the context only when every one exists, so a
+        // failure half-way leaves the context as it was and the next call tries again
+        cudaStream_t qs[2] = {nullptr, nullptr};
+        cudaEvent_t qe[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+        cudaError_t qerr = cudaSuccess;
+        for (int k = 0; k < 2 && qerr == cudaSuccess; ++k) qerr = cudaStreamCreateWithFlags(&qs[k], cudaStreamNonBlocking);
+        for (int k = 0; k < 6 && qerr == cudaSuccess; ++k) qerr = cudaEventCreateWithFlags(&qe[k], cudaEventDisableTiming);
+        if (qerr != cudaSuccess) {
+            for (cudaStream_t q : qs)
+                if (q) cudaStreamDestroy(q);
+            for (cudaEvent_t q : qe)
+                if (q) cudaEventDestroy(q);
+            return fail(DEMONS_E_CUDA, "creating the queue's streams and events failed: %s", cudaGetErrorString(qerr));
+        }
+        c->q_in = qs[0];
+        c->q_out = qs[1];
         for (int k = 0; k < 2; ++k) {
-            CUDA_TRY(cudaEventCreateWithFlags(&c->q_up[k], cudaEventDisableTiming));
-            CUDA_TRY(cudaEventCreateWithFlags(&c->q_done[k], cudaEventDisableTiming));
-            CUDA_TRY(cudaEventCreateWithFlags(&c->q_down[k], cudaEventDisableTiming));
+            c->q_up[k] = qe[3 * k];
+            c->q_done[k] = qe[3 * k + 1];
+            c->q_down[k] = qe[3 * k + 2];
         }
     }
     const Partition p = make_partition(c, levels, 1);

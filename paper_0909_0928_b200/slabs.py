@@ -122,11 +122,23 @@ class DistExchange:
 
 
 def iterate_slabs(engines, slabs, dS, dM, fields, scratch, iters, sigma, exchange, metrics=None, fields_b=None,
-                  scratch_b=None):
+                  scratch_b=None, eps=0.0):
     """`iters` iterations on the slabs in `fields` (a list with one entry per rank this process holds; one entry
     under torch.distributed).  engines[i]: binding.Demons created with the WHOLE volume's dims; metrics (optional):
     float64 device tensors (iters, 3) per held rank, filled with the sums over own planes.  Everything is enqueued
-    on torch's current stream, so that kernels, halo copies and NCCL transfers are ordered."""
+    on torch's current stream, so that kernels, halo copies and NCCL transfers are ordered.
+
+    Limits, checked here: exactly `iters` iterations run -- the stopping rule of PAPER.md L145 needs the three sums
+    added over all ranks after every iteration, which this loop does not do, so eps > 0 is refused rather than
+    ignored; and every slab must carry a halo of at least halo_planes(sigma) planes (plan() has already refused
+    splits in which a rank owns fewer planes than its halo, i.e. world > nz / halo)."""
+    if eps is not None and float(eps) > 0.0:
+        raise ValueError("iterate_slabs runs fixed iteration counts: the stopping rule (eps > 0) needs the metrics "
+                         "summed over the ranks every iteration, which the slab loop does not do")
+    need = halo_planes(sigma)
+    for s in slabs:
+        if s.world > 1 and s.halo < need:
+            raise ValueError(f"slab of rank {s.rank} has a halo of {s.halo} planes; sigma = {sigma} needs {need}")
     import torch
     dims = engines[0].dims
     local = isinstance(exchange, LocalExchange)

@@ -351,9 +351,11 @@ def run_register_batch(torch, B, variant, pairs, iters, alpha=1.0, eps=0.0, opti
 
 
 @pytest.mark.parametrize("variant", [0, 1, 3, 5])
-def test_register_batch_equals_single_calls(torch_cuda, B, P, variant):
+def test_register_batch_equals_single_calls(torch_cuda, B, P, oracle, variant):
     """demons_register_batch: every pair of the batch gets the field demons_register gives it alone, bit for
-    bit; the statistics agree to rounding (the block partition of the reduction differs with the batch)."""
+    bit; the statistics agree to rounding (the block partition of the reduction differs with the batch).  The first
+    and the last pair are also compared with the oracle's registration, so that a fault common to both CUDA arms
+    cannot pass."""
     dims = (44, 36, 22)
     iters = [9, 7, 6]
     pairs = [P.config1_pair(dims=dims, seed=300 + k, max_norm=1.5 + 0.3 * k)[:2] for k in range(5)]
@@ -367,7 +369,76 @@ def test_register_batch_equals_single_calls(torch_cuda, B, P, variant):
             assert np.array_equal(ub[k], one["ub"])
         np.testing.assert_allclose(stats[k], one["stats"], rtol=1e-12, atol=0)
         assert done[k].tolist() == one["iters_done"]
+        if k in (0, len(pairs) - 1):
+            ref = oracle.register(variant, ALPHA.get(variant, 1.0), 1.0, S, M, iters)
+            check_registration(dict(u=u[k], ub=ub[k] if variant == 5 else None, stats=stats[k],
+                                    iters_done=done[k].tolist()), ref, f"batch pair {k} vs oracle")
     assert launches <= 1.1 * singles / len(pairs)    # every level small enough to run as ONE group: a single registration's launch count
+
+
+def test_single_call_after_batch_on_one_context(torch_cuda, B):
+    """One context, one workspace sized for a batch: a batch of two on a level large enough to run pair by pair
+    (3 Mvoxel), then a single registration on the SAME buffers of pair 0.  The cached level graph of the batch carries
+    workspace offsets laid out for two pairs; the single call must not replay it (its statistics and, for variant 1,
+    its |grad M|^2 live at the offsets of a one-pair layout).  Field and statistics must equal a fresh context's."""
+    torch = torch_cuda
+    dims = (192, 128, 128)
+    shape = (dims[2], dims[1], dims[0])
+    z, y, x = torch.meshgrid(*[torch.arange(n, dtype=torch.float32, device="cuda:0") for n in shape], indexing="ij")
+    S0 = 100.0 * torch.sin(0.11 * x) * torch.cos(0.07 * y) + 60.0 * torch.sin(0.09 * z + 0.05 * x)
+    M0 = 100.0 * torch.sin(0.11 * (x + 1.3)) * torch.cos(0.07 * (y - 0.8)) + 60.0 * torch.sin(0.09 * (z + 0.9) + 0.05 * x)
+    dS = torch.stack([S0, S0 * 0.9 + 5.0]).contiguous()
+    dM = torch.stack([M0, M0 * 0.9 + 5.0]).contiguous()
+    iters = [8]
+    st = torch.cuda.Stream()
+    for variant in (0, 1):
+        eng = B.Demons(dims, variant=variant, levels=1, nbatch=2)
+        du = torch.zeros((2, 3) + shape, dtype=torch.float32, device="cuda:0")
+        torch.cuda.synchronize()
+        B.demons_register_batch(eng.ctx, 2, dS, dM, du, None, iters, 0.0, None, None, st)
+        torch.cuda.synchronize()
+        batch_u0 = du[0].clone()
+        du.zero_()
+        stats = np.zeros((8, 3))
+        torch.cuda.synchronize()
+        B.demons_register(eng.ctx, dS[0], dM[0], du[0], None, iters, 0.0, stats, None, st)
+        torch.cuda.synchronize()
+        after_batch = du[0].clone()
+        eng.close()
+        fresh = B.Demons(dims, variant=variant, levels=1)
+        du2 = torch.zeros((3,) + shape, dtype=torch.float32, device="cuda:0")
+        stats2 = np.zeros((8, 3))
+        torch.cuda.synchronize()
+        B.demons_register(fresh.ctx, dS[0], dM[0], du2, None, iters, 0.0, stats2, None, st)
+        torch.cuda.synchronize()
+        fresh.close()
+        assert float(du2.abs().max()) > 0.1 and stats2[:, 0].min() > 0
+        assert torch.equal(after_batch, du2), f"variant {variant}: single call after a batch differs from a fresh context"
+        assert torch.equal(batch_u0, du2)
+        np.testing.assert_allclose(stats, stats2, rtol=1e-12, atol=0)
+
+
+def test_register_batch_thin_tall_level(torch_cuda, B):
+    """6 x 6 x 4000: nx % 4 != 0 sends the level to the separable smoothing passes and the scalar |grad M|^2 kernel,
+    which carry planes x components x pairs in gridDim.z.  A batch of 12 would need 144 000 there; the driver must
+    split the batch into groups that fit instead of failing where every pair alone succeeds."""
+    rng = np.random.default_rng(77)
+    shape = (4000, 6, 6)
+    zz = np.arange(shape[0], dtype=np.float32)[:, None, None]
+    pairs = []
+    for k in range(12):
+        S = (100.0 * np.sin(0.05 * zz + k) + 10.0 * rng.standard_normal(shape)).astype(np.float32)
+        M = (100.0 * np.sin(0.05 * (zz + 0.7) + k) + 10.0 * rng.standard_normal(shape)).astype(np.float32)
+        pairs.append((S, M))
+    iters = [2, 3]
+    for variant in (0, 1):
+        u, _, stats, done, _ = run_register_batch(torch_cuda, B, variant, pairs, iters)
+        for k in (0, 7, 11):
+            one = run_register(torch_cuda, B, variant, pairs[k][0], pairs[k][1], iters)
+            assert np.array_equal(u[k], one["u"]), f"variant {variant} pair {k}"
+            np.testing.assert_allclose(stats[k], one["stats"], rtol=1e-12, atol=0)
+            assert done[k].tolist() == one["iters_done"]
+        assert np.abs(u).max() > 1e-3
 
 
 def test_register_batch_groups_and_early_stop(torch_cuda, B, P, oracle):
@@ -381,6 +452,9 @@ def test_register_batch_groups_and_early_stop(torch_cuda, B, P, oracle):
     for k, (S, M) in enumerate(pairs):
         one = run_register(torch, B, 0, S, M, iters)
         assert np.array_equal(u[k], one["u"]), f"pair {k}"
+        if k in (0, 3):   # one pair of the group of three, and the pair that runs alone: against the oracle
+            check_registration(dict(u=u[k], ub=None, stats=stats[k], iters_done=done[k].tolist()),
+                               oracle.register(0, 1.0, 1.0, S, M, iters), f"grouped batch pair {k} vs oracle")
     # early stop, small volumes: different pairs stop at different iterations
     dims = (32, 32, 16)
     pairs = [P.config1_pair(dims=dims, seed=9 + k, noise_sd=0.0, max_norm=1.0 + 0.4 * k)[:2] for k in range(4)]
@@ -394,11 +468,13 @@ def test_register_batch_groups_and_early_stop(torch_cuda, B, P, oracle):
         n = one["iters_done"][0]
         assert np.all(stats[k, n:] == 0.0)
         stops.append(n)
+        check_registration(dict(u=u[k], ub=None, stats=stats[k], iters_done=done[k].tolist()),
+                           oracle.register(0, 1.0, 1.0, S, M, [60], eps=eps), f"early-stop batch pair {k} vs oracle")
     assert len(set(stops)) > 1 and min(stops) < 60, stops
 
 
 @pytest.mark.parametrize("variant", [0, 3])
-def test_register_batch_sigma2_shares_and_early_stop(torch_cuda, B, P, variant):
+def test_register_batch_sigma2_shares_and_early_stop(torch_cuda, B, P, oracle, variant):
     """sigma = 2 (R = 6): the smoothing kernel splits the columns of ALL pairs into equal shares of one wave, so a CTA's
     run of planes crosses from one component / pair into the next, and the stop flag is tested per segment.  The batch
     still equals the single registrations bit for bit, with eps > 0 stopping every pair on its own iteration."""
@@ -416,11 +492,14 @@ def test_register_batch_sigma2_shares_and_early_stop(torch_cuda, B, P, variant):
         assert done[k].tolist() == one["iters_done"]
         np.testing.assert_allclose(stats[k], one["stats"], rtol=1e-12, atol=0)
         stops.append(one["iters_done"][0])
+        if k in (0, 4):
+            check_registration(dict(u=u[k], ub=None, stats=stats[k], iters_done=done[k].tolist()),
+                               oracle.register(variant, alpha, 2.0, S, M, [50], eps=eps), f"sigma-2 batch pair {k} vs oracle")
     assert min(stops) >= 10, stops
 
 
 @pytest.mark.parametrize("variant,levels", [(0, 1), (3, 2), (5, 2)])
-def test_register_host_queue_equals_single_host_calls(torch_cuda, B, P, variant, levels):
+def test_register_host_queue_equals_single_host_calls(torch_cuda, B, P, oracle, variant, levels):
     """demons_register_host_queue: n registrations from pinned host buffers with the transfers of neighbouring
     registrations overlapped; every field, statistics row and iteration count equals the demons_register_host call on
     that pair, bit for bit (two staging slots: five pairs go round the slots more than twice)."""
@@ -454,6 +533,11 @@ def test_register_host_queue_equals_single_host_calls(torch_cuda, B, P, variant,
             assert np.array_equal(hUb[k].numpy(), hub), f"pair {k} (backward field)"
         assert np.array_equal(stats[k], s1) and done[k].tolist() == d1.tolist()
         assert np.abs(hu).max() > 0
+        if k in (0, 4):   # first pair and the pair that has gone round both staging slots twice: against the oracle
+            ref = oracle.register(variant, alpha, 1.0, S, M, iters, u0=u0[k] if levels == 1 else None,
+                                  ub0=-u0[k] if ic and levels == 1 else None)
+            check_registration(dict(u=hU[k].numpy(), ub=hUb[k].numpy() if ic else None, stats=stats[k],
+                                    iters_done=done[k].tolist()), ref, f"queue pair {k} vs oracle")
     eng.close()
 
 
@@ -495,7 +579,7 @@ def test_inverse_consistent_one_field_is_bit_identical(torch_cuda, B, P, oracle)
 
 @pytest.mark.parametrize("variant,world,levels,one_field", [(0, 3, 1, 0), (1, 2, 1, 0), (2, 3, 1, 0), (3, 2, 2, 0), (5, 2, 1, 0),
                                                           (5, 3, 2, 1), (0, 4, 2, 0)])
-def test_z_slab_decomposition_is_bit_identical(torch_cuda, B, P, variant, world, levels, one_field):
+def test_z_slab_decomposition_is_bit_identical(torch_cuda, B, P, oracle, variant, world, levels, one_field):
     """the registration split into z slabs (own planes + R + 1 halo planes, images replicated, one
     halo refresh per iteration; paper_0909_0928_b200/slabs.py) gives on every rank's own planes the bits of the
     undivided registration.  The ranks are emulated one after another on this GPU; their halos move through
@@ -520,6 +604,10 @@ def test_z_slab_decomposition_is_bit_identical(torch_cuda, B, P, variant, world,
     B.demons_register(eng.ctx, dS, dM, du, dub, iters, 0.0, stats, None, None)
     torch.cuda.synchronize()
     eng.close()
+    # the undivided registration itself against the oracle, on the whole volume
+    ref = oracle.register(variant, alpha, sigma, S, M, iters)
+    check_registration(dict(u=du.cpu().numpy(), ub=dub.cpu().numpy() if ic else None, stats=stats,
+                            iters_done=ref["iters_done"]), ref, "undivided registration vs oracle")
     # the same in `world` slabs
     plan = SL.plan(dims[2], world, SL.halo_planes(sigma))
     assert plan[0].lo == 0 and plan[-1].hi == dims[2] and all(a.own1 == b.own0 for a, b in zip(plan, plan[1:]))
@@ -549,6 +637,99 @@ def test_z_slab_decomposition_is_bit_identical(torch_cuda, B, P, variant, world,
     np.testing.assert_allclose(total, stats[-iters[-1]:], rtol=1e-12)
     for e in engines:
         e.close()
+
+
+def _nccl_slab_worker(rank, world, port, variant, out):
+    """One rank of the two-GPU slab test: its own GPU, NCCL halo exchange, compared with the undivided registration
+    computed on the same GPU."""
+    import os
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port))
+    import torch
+    import torch.distributed as dist
+    from paper_0909_0928_b200 import binding as B, phantoms as P, slabs as SL
+    device = f"cuda:{rank}"
+    torch.cuda.set_device(rank)
+    dist.init_process_group("nccl", rank=rank, world_size=world)
+    try:
+        dims, sigma, iters = (64, 40, 44), 1.0, 6
+        S, M, _ = P.config1_pair(dims=dims, seed=55, max_norm=2.5)
+        dS = torch.from_numpy(np.ascontiguousarray(S)).to(device)
+        dM = torch.from_numpy(np.ascontiguousarray(M)).to(device)
+        eng = B.Demons(dims, variant=variant, sigma=sigma, levels=1, device=device)
+        B.demons_set_option(eng.ctx, "zero_start", 1)
+        du = torch.zeros((3,) + S.shape, dtype=torch.float32, device=device)
+        stats = np.zeros((iters, 3))
+        B.demons_register(eng.ctx, dS, dM, du, None, [iters], 0.0, stats, None, None)
+        torch.cuda.synchronize()
+        eng.close()
+        s = SL.plan(dims[2], world, SL.halo_planes(sigma))[rank]
+        slab_eng = B.Demons(dims, variant=variant, sigma=sigma, levels=1, device=device)
+        field = torch.zeros((3, s.count) + S.shape[1:], dtype=torch.float32, device=device)
+        scratch = torch.empty_like(field)
+        metrics = torch.zeros((iters, 3), dtype=torch.float64, device=device)
+        SL.iterate_slabs([slab_eng], [s], dS, dM, [field], [scratch], iters, sigma, SL.DistExchange(s), [metrics])
+        dist.all_reduce(metrics)
+        torch.cuda.synchronize()
+        same = bool(torch.equal(field[:, s.own_begin:s.own_begin + s.own_count], du[:, s.own0:s.own1]))
+        close = bool(np.allclose(metrics.cpu().numpy(), stats, rtol=1e-12, atol=0))
+        slab_eng.close()
+        out.put((rank, same, close))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("variant", [0, 2])
+def test_z_slabs_over_nccl_on_two_gpus(torch_cuda, variant):
+    """The slab loop with DistExchange over NCCL, one process per GPU: own planes carry the bits of the undivided
+    registration and the all-reduced metrics its statistics.  Needs two GPUs (skipped on a one-GPU box, where
+    test_z_slab_decomposition_is_bit_identical covers the same arithmetic with emulated ranks)."""
+    torch = torch_cuda
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    import multiprocessing as mp
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_nccl_slab_worker, args=(r, 2, port, variant, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=300) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert res == [(0, True, True), (1, True, True)]
+
+
+def test_in_graph_timing_changes_no_bits(torch_cuda, B, P):
+    """"profile" = 2: event-record nodes inside the replayed level graph.  Same field as the untimed run, one timed
+    iteration per replayed 20-chunk (45 iterations = 2 replays + 5 single iterations), positive durations, and the
+    option can be switched off again."""
+    torch = torch_cuda
+    S, M, _ = P.config1_pair()
+    dims = (S.shape[2], S.shape[1], S.shape[0])
+    dS, dM = dev(torch, S), dev(torch, M)
+    st = torch.cuda.Stream()
+    for variant in (0, 3):
+        eng = B.Demons(dims, variant=variant, levels=1)
+        B.demons_set_option(eng.ctx, "zero_start", 1)
+        outs = []
+        for prof in (0, 2, 0):
+            B.demons_set_option(eng.ctx, "profile", prof)
+            du = torch.full((3,) + S.shape, 9.0, dtype=torch.float32, device="cuda:0")
+            torch.cuda.synchronize()
+            B.demons_register(eng.ctx, dS, dM, du, None, [45], 0.0, None, None, st)
+            torch.cuda.synchronize()
+            outs.append(du)
+            if prof == 2:
+                got = B.demons_get_profile(eng.ctx)
+                assert got["force"]["groups"] == 2 and got["smooth"]["groups"] == 2
+                assert 0.0 < got["force"]["ms"] < 50.0 and 0.0 < got["smooth"]["ms"] < 50.0
+        assert torch.equal(outs[0], outs[1]) and torch.equal(outs[0], outs[2])
+        eng.close()
 
 
 def test_api_rejects_bad_calls(torch_cuda, B):

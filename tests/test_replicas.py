@@ -86,6 +86,19 @@ def test_slab_plan_covers_the_volume():
         SL.plan(12, 4, 4)                                # 3 planes per rank cannot fill a 4-plane halo
 
 
+def test_slab_loop_refuses_what_it_cannot_do():
+    """iterate_slabs: eps > 0 (the stopping rule needs an all-reduce per iteration) and a halo thinner than the
+    smoothing radius + 1 are refused before any kernel is launched."""
+    from paper_0909_0928_b200 import slabs as SL
+    plan = SL.plan(40, 2, SL.halo_planes(1.0))
+    with pytest.raises(ValueError, match="stopping rule"):
+        SL.iterate_slabs([], plan, None, None, [], [], 5, 1.0, SL.LocalExchange(plan), eps=1e-4)
+    with pytest.raises(ValueError, match="halo"):
+        SL.iterate_slabs([], plan, None, None, [], [], 5, 2.0, SL.LocalExchange(plan))
+    with pytest.raises(ValueError, match="fewer than the halo"):
+        SL.plan(256, 64, SL.halo_planes(2.0))            # 512x512x256 on 64 ranks at sigma 2: 4 planes < halo 7
+
+
 def _slab_worker(rank, world, port, out):
     os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), MASTER_ADDR="127.0.0.1",
                       MASTER_PORT=str(port))
