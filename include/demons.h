@@ -21,6 +21,13 @@
  *  - Every function returns a DEMONS_* status; nothing throws, aborts or exits.  On failure
  *    demons_last_error() returns a thread-local description.  There is no CPU fallback: with no
  *    usable CUDA device every compute entry point returns DEMONS_E_CUDA.
+ *  - ONE DEVICE-WIDE SIDE EFFECT, on by default: with the "l2_persist" option (default 1) the first call that gathers
+ *    from a moving image raises the device limit cudaLimitPersistingL2CacheSize to that image's size (other users of
+ *    the device see a smaller non-persisting L2 while lines are pinned); demons_destroy resets the persisting lines
+ *    and restores the limit it found.  demons_set_option(ctx, "l2_persist", 0) before the first compute call leaves
+ *    the device untouched (the fused pass is then ~10 % slower at 256x256x100).  Details under demons_set_option.
+ *  - Host threads: entry points may be called from several host threads as long as each context is used by one
+ *    thread at a time; the library's per-device one-time set-up is synchronised, the error string is per thread.
  *  - Buffers that are 16-byte aligned with nx % 4 == 0 take the fast kernels (TMA-fed smoothing, 128-bit
  *    rows in the stencil pass; the gathering passes use lane-consecutive 32-bit accesses, one 128-byte
  *    line per warp); anything else takes scalar kernels with identical results.

@@ -26,6 +26,7 @@
 // wrote last are read first while they are still in L2, and the planes written last here are the
 // ones the next force kernel reads first.  The taps are symmetric: the result is bit-identical.
 #include <algorithm>
+#include <atomic>
 
 #include "kernels.h"
 #include "tma.cuh"
@@ -418,17 +419,19 @@ int launch_cfg(const SmoothArgs& a, int slots, cudaStream_t st) {
                                         (unsigned long long)a.ncomp};
     const unsigned box[4] = {(unsigned)C::BOXW, (unsigned)C::ROWS, 1u, 1u};
     if (!tma::encode_f32(&map, a.in, 4, gdim, box)) return 0;
-    static bool attr_set[64] = {};  // per device: the attribute belongs to the device's copy of the kernel
+    // per device: the attribute belongs to the device's copy of the kernel.  Atomic flags: two host threads may get
+    // here together; setting the attribute twice is harmless, a torn flag is not.
+    static std::atomic<bool> attr_set[64] = {};
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 0;
-    if (!attr_set[dev]) {
+    if (!attr_set[dev].load(std::memory_order_acquire)) {
         if (cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES, MINB, PAIR, XP, BAL>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM) !=
             cudaSuccess) {
             cudaGetLastError();
             return 0;  // refused: not applicable here, the caller falls back to the separable passes
         }
         cudaFuncSetAttribute(k_smooth_tma<R, K, RG, STAGES, MINB, PAIR, XP, BAL>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-        attr_set[dev] = true;
+        attr_set[dev].store(true, std::memory_order_release);
     }
     const int tiles_x = (d.nx + C::GX * 4 - 1) / (C::GX * 4);
     const int tiles_y = (d.ny + C::TY - 1) / C::TY;

@@ -16,6 +16,8 @@
 //
 // Every kernel carries a pair index in blockIdx.z (blockIdx.z = pair * chunks + z-chunk): a batch of
 // independent registrations runs as ONE launch per kernel, so that the small pyramid levels fill the GPU.
+#include <mutex>
+
 #include "kernels.h"
 
 namespace demons {
@@ -900,6 +902,8 @@ struct DeviceProps {
 
 const DeviceProps& device_props() {
     static DeviceProps props[64];
+    static std::mutex props_mutex;  // host threads driving different contexts share this table
+    std::lock_guard<std::mutex> lock(props_mutex);
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) {
         cudaGetLastError();

@@ -170,6 +170,29 @@ def lung_pair(dims=(256, 256, 100), seed=202):
     return S, M, d
 
 
+def textured_pair(dims=(256, 256, 100), seed=212, max_d=2.0):
+    """A WELL-CONDITIONED full-size pair: an analytic texture with intensity gradient almost everywhere (three oblique
+    sinusoids, amplitudes of CT-like size), S = tex(x), M = tex(x + d) evaluated analytically for a smooth known field
+    d of at most `max_d` voxels (bumps of width 20-40 voxels).  On the lung phantom -- with or without noise, with or
+    without softened edges -- large regions are flat, the force there is 0/0-like (d ~ 0, grad ~ 0) and rounding
+    differences grow to tenths of a voxel over a registration; here the oracle differs from itself by ~2e-6 voxel when
+    the input moves by one ulp, so the END state of a full registration can be held to north_star's plain 1e-2 voxel
+    bar.  Returns (S, M, d)."""
+    rng = np.random.default_rng(seed)
+    nx, ny, nz = dims
+    z, y, x = np.meshgrid(np.arange(nz, dtype=np.float64), np.arange(ny, dtype=np.float64),
+                          np.arange(nx, dtype=np.float64), indexing="ij")
+
+    def tex(px, py, pz):
+        return (100.0 * np.sin(0.31 * px + 0.05 * pz) * np.cos(0.23 * py) + 60.0 * np.sin(0.27 * pz + 0.11 * px + 0.07 * py)
+                + 40.0 * np.cos(0.19 * px - 0.29 * py + 0.13 * pz))
+
+    d = bump_field(dims, rng, 8, (20.0, 40.0), max_d, centre_frac=1.0)
+    S = tex(x, y, z).astype(np.float32)
+    M = tex(x + d[0], y + d[1], z + d[2]).astype(np.float32)
+    return S, M, d
+
+
 def sweep_inputs(dims, seed):
     """BASELINE.json config 5: blob static, random smooth u (32 bumps, widths U[8,24],
     max |u| = 8 voxels), moving = static resampled by a second such field.  Returns (S, M, u)."""

@@ -1,18 +1,21 @@
 """BASELINE.json config 5: bandwidth sweep of the per-iteration kernels through the C ABI.
 
-    python -m paper_0909_0928_b200.sweep [--sizes 128x128x64,256x256x100,...] [--reps 20]
-                                         [--kernels force,iteration,smooth,pyramid,texture] [--json out.json]
+    python sweep.py [--sizes 128x128x64,256x256x100,...] [--reps 20] [--batch B]
+                    [--kernels force,iteration,smooth,pyramid,texture] [--json out.json]
 
 For every size: the fused warp+force+update entry point for all six variants, the Gaussian
 smoothing at sigma 1.0 and 2.0 (3 components), restrict and prolong.  Inputs are the seeded blob
 phantom and a random smooth field with max |u| = 8 voxels (phantoms.sweep_inputs).  `iteration[...]` rows time one
-whole [force ; smooth] iteration inside a registration (40 iterations, one level, sigma 1).  Reported per
+whole [force ; smooth] iteration inside a registration (40 iterations, one level, sigma 1); with --batch B > 1 the
+passive and double-force iteration rows are repeated through demons_register_batch with B pairs per call (time per
+pair: what the batch axis does for sizes whose launches cannot fill 148 SMs).  Reported per
 kernel: median over `reps` samples of 10 back-to-back launches (CUDA events) after 3 warm-ups, effective GB/s = algorithmic
 bytes (DESIGN.md byte table) / time, and % of the measured HBM peak.  The same command with
 --reps 1 --warmups 1 --inner 1 (every entry point launched twice) is what the ncu captures under profiles/ run.  S and M are separate allocations here, so the L2
 access-policy window of the gathering kernels covers M alone (bench.py's pair shares one allocation and
 gets both images).  The CPU oracle's time per call for the same entry points is measured by bench.py's
-cpu_baseline leg (this package never loads the oracle).
+cpu_baseline leg (this script never loads the oracle).  A measurement script, like bench.py: it sits beside it, not
+in the library package.
 """
 from __future__ import annotations
 
@@ -24,7 +27,7 @@ import time
 
 import numpy as np
 
-ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+ROOT = os.path.dirname(os.path.abspath(__file__))
 SEEDS = {(128, 128, 64): 500, (256, 256, 100): 501, (512, 512, 160): 502, (512, 512, 256): 503}
 # algorithmic bytes per voxel of each entry point as implemented
 # variant 1 through the standalone entry point: |grad M|^2 pass (4 in, 4 out) + fused pass (u 12, S 4, M 4,
@@ -64,10 +67,10 @@ def median_ms(torch, stream, fn, reps, inner=None):
     return float(np.median(times))
 
 
-def run(sizes, kernels, reps, device="cuda:0"):
+def run(sizes, kernels, reps, device="cuda:0", batch=1):
     import torch
-    from . import binding as B
-    from . import build, phantoms
+    from paper_0909_0928_b200 import binding as B
+    from paper_0909_0928_b200 import build, phantoms
     build.build()
     B.lib()
     peak, peak_kind = hbm_peak()
@@ -143,6 +146,22 @@ def run(sizes, kernels, reps, device="cuda:0"):
                 fb = {0: 32.0, 1: 36.0, 2: 52.0, 3: 52.0, 4: 52.0, 5: 96.0}[variant]
                 add(f"iteration[{VARIANT_NAMES[variant]}]", ms, (fb + (48.0 if ic else 24.0)) * N)
                 eng.close()
+            if batch > 1 and batch * N < (1 << 29):
+                # the same iteration with `batch` pairs per call (demons_register_batch): ms per pair and iteration
+                bS = torch.stack([torch.roll(dS, k, dims=2) for k in range(batch)]).contiguous()
+                bM = torch.stack([torch.roll(dM, k, dims=2) for k in range(batch)]).contiguous()
+                bu0 = torch.stack([torch.roll(du, k, dims=3) for k in range(batch)]).contiguous()
+                bu = torch.empty_like(bu0)
+                for variant in (0, 3):
+                    eng = B.Demons(dims, variant=variant, sigma=1.0, device=device, nbatch=batch)
+                    bu.copy_(bu0)
+                    torch.cuda.synchronize()
+                    ms = median_ms(torch, stream, lambda: B.demons_register_batch(
+                        eng.ctx, batch, bS, bM, bu, None, [its], 0.0, None, None, stream), max(3, reps // 4), inner=1) / (its * batch)
+                    fb = {0: 32.0, 3: 52.0}[variant]
+                    add(f"iteration[{VARIANT_NAMES[variant]}, B={batch}]", ms, (fb + 24.0) * N)
+                    eng.close()
+                del bS, bM, bu0, bu
     return rows, peak, peak_kind
 
 
@@ -152,13 +171,14 @@ def main():
     ap.add_argument("--kernels", default="force,iteration,smooth,pyramid,texture")
     ap.add_argument("--reps", type=int, default=20)
     ap.add_argument("--json", default=None)
+    ap.add_argument("--batch", type=int, default=1, help="also time the iteration rows with this many pairs per call")
     ap.add_argument("--warmups", type=int, default=3)
     ap.add_argument("--inner", type=int, default=10, help="back-to-back launches per timed sample")
     args = ap.parse_args()
     global WARMUPS, INNER
     WARMUPS, INNER = args.warmups, args.inner
     sizes = [tuple(int(v) for v in s.split("x")) for s in args.sizes.split(",")]
-    rows, peak, kind = run(sizes, set(args.kernels.split(",")), args.reps)
+    rows, peak, kind = run(sizes, set(args.kernels.split(",")), args.reps, batch=args.batch)
     print(f"# HBM peak {peak:.1f} GB/s ({kind}); effective GB/s = algorithmic bytes / median time")
     print(f"{'dims':>12} {'kernel':<34} {'ms':>9} {'GB/s':>9} {'% peak':>7} {'% 8TB/s':>8}")
     for r in rows:
@@ -174,5 +194,4 @@ def main():
 
 
 if __name__ == "__main__":
-    sys.path.insert(0, ROOT)
     main()

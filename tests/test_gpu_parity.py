@@ -732,6 +732,42 @@ def test_in_graph_timing_changes_no_bits(torch_cuda, B, P):
         eng.close()
 
 
+def test_two_host_threads_two_contexts(torch_cuda, B, P):
+    """The header promises a thread-local error string, so host threads are an expected use: two threads, each with
+    its own context, workspace and stream on the same device, register different pairs at the same time (ctypes
+    releases the GIL during the calls); each result equals the one the pair gives alone, bit for bit.  Fresh sigma /
+    size combinations, so that the per-device one-time set-up inside the library is reached by both threads."""
+    import threading
+    torch = torch_cuda
+    dims = (72, 56, 28)
+    pairs = [P.config1_pair(dims=dims, seed=900 + k, max_norm=1.5)[:2] for k in range(2)]
+    variants = [0, 3]
+    sigma = 1.4          # R = 5: a smoother instantiation the other tests of this file do not use first
+    iters = [12, 10]
+    rounds = []
+    for _ in range(3):
+        got, errs = [None, None], []
+
+        def work(k):
+            try:
+                got[k] = run_register(torch, B, variants[k], pairs[k][0], pairs[k][1], iters, sigma=sigma)
+            except Exception as e:          # noqa: BLE001 -- reported below
+                errs.append(e)
+
+        ts = [threading.Thread(target=work, args=(k,)) for k in range(2)]
+        for t in ts:
+            t.start()
+        for t in ts:
+            t.join()
+        assert not errs, errs
+        rounds.append(got)
+    want = [run_register(torch, B, variants[k], pairs[k][0], pairs[k][1], iters, sigma=sigma) for k in range(2)]
+    for got in rounds:
+        for k in range(2):
+            assert np.array_equal(got[k]["u"], want[k]["u"]), f"thread {k}"
+            np.testing.assert_array_equal(got[k]["stats"], want[k]["stats"])
+
+
 def test_api_rejects_bad_calls(torch_cuda, B):
     torch = torch_cuda
     dims = (16, 16, 8)
